@@ -1,0 +1,132 @@
+/*
+ * lise.h -- C-ABI boundary of the B200-native TDSLDA time-step library (liblise.so).
+ *
+ * One thing is built here: the data-parallel hot path of arxiv/paper_2009_00745 (the LISE package) --
+ * the TDSLDA right-hand side and the Adams-Bashforth-Milne (ABM) step applied to every quasiparticle
+ * wavefunction (qpwf) on a periodic 3D lattice.  All arithmetic is IEEE fp64 (complex128) in
+ * hand-written CUDA kernels for sm_100a; there is no CPU fallback and no cuFFT/cuBLAS on this path.
+ * Citations are "PAPER.md:L<line>" of the paper text plus equation numbers; the adopted reading of
+ * every garbled or ambiguous passage is listed in DESIGN.md (ledger B1..B27).
+ *
+ * Conventions
+ *   species     0 = neutrons, 1 = protons; nwf_p = 0 means neutrons only (Coulomb then off).
+ *   lattice     nx, ny, nz even; lattice constant dx = dy = dz (Eq. 43); volume element dV = dx^3.
+ *   wavefunction block ("psi"): [state][component: u_up, u_dn, v_up, v_dn][ix][iy][iz], iz fastest,
+ *               interleaved (re, im) doubles (Eq. 1; the order inside xyz is this library's choice).
+ *               States are normalised as dV * sum |psi|^2 = 1, so densities are in fm^-3.
+ *   pointers    every `*_dev` argument is a DEVICE pointer owned by the caller (e.g. a torch tensor);
+ *               the library reads/writes it on the context's stream and never frees or retains it.
+ *               Every other pointer is a HOST pointer.
+ *   ordering    calls enqueue work on the context's stream and return without synchronising, except
+ *               lise_observables (synchronises, writes host memory) and lise_create / lise_destroy.
+ *   errors      every call returns LISE_OK (0) or a negative LISE_E* code; nothing throws or aborts.
+ *               lise_last_error(ctx) gives a human-readable message for the last failure.
+ *   units       MeV, fm, fm/c.
+ */
+#ifndef LISE_H
+#define LISE_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+    LISE_OK = 0,
+    LISE_EINVAL = -1,       /* bad argument (null pointer, odd lattice size, species out of range ...) */
+    LISE_ESTATE = -2,       /* call order: wavefunctions of a species not set yet                      */
+    LISE_ECUDA = -3,        /* a CUDA runtime call or kernel launch failed                             */
+    LISE_ENOMEM = -4,       /* device memory allocation failed                                         */
+    LISE_EUNSUPPORTED = -5  /* lattice too large for the on-chip plane tiles of this build             */
+};
+
+typedef struct lise_ctx lise_ctx; /* opaque; owns every internal device buffer */
+
+/* Physical parameters.  None is printed in the paper; defaults (lise_default_params) are SLy4
+ * (the paper's default force) and volume pairing with the cubic-cutoff
+ * renormalisation of Eq. 21. */
+typedef struct {
+    double hbar2_2m, e2, hbarc;                         /* 20.73553 MeV fm^2, 1.439964 MeV fm, 197.3269804 MeV fm */
+    double t0, t1, t2, t3, x0, x1, x2, x3, gamma, W0;   /* Skyrme parameters -> couplings of Eq. 9               */
+    double g0_n, g0_p;                                  /* bare pairing couplings, MeV fm^3 (0 = pairing off)    */
+    int coulomb;                                        /* 1: Coulomb direct (Eqs. 58-62) + Slater exchange (Eq. 6) for protons */
+    int pairing_rearrangement;                          /* 1: include d E_pair / d n in U (reading B8) */
+    int remove_phase;                                   /* 1: subtract eta_k = <psi_k|H|psi_k> (Eqs. 80-81)      */
+} lise_params;
+
+/* Observables of the current wavefunctions y_n (E(t), Z(t), N(t)). */
+typedef struct {
+    double energy, e_kin, e_skyrme, e_coul, e_pair;     /* Eq. 4 and its parts (Eqs. 5-9), MeV               */
+    double n_neutron, n_proton;                         /* dV * sum n_q                                      */
+    double norm_defect;                                 /* max_k | <psi_k|psi_k> - 1 |                       */
+    double ortho_defect;                                /* max over pairs (k, (k+d) mod nwf), d in {1, 2, nwf/2}, of |<psi_k|psi_l>| */
+    double time;                                        /* fm/c                                              */
+    long step;                                          /* steps taken since the last lise_set_wavefunctions */
+} lise_observables_t;
+
+int lise_default_params(lise_params *p);
+
+/* Allocates a context for an nx x ny x nz lattice with spacing dx (fm), time step dt (fm/c) and
+ * nwf_n / nwf_p quasiparticle states.  Device memory: 7 state arrays per species
+ * (y_n, y_{n-1}, three f = dy/dt history arrays, e_n = p_n - c_n, predictor scratch; the paper's
+ * code holds 11, Eq. 83) plus a chunk-sized H psi scratch and grid fields.  Uses the current CUDA
+ * device and the legacy default stream until lise_set_stream is called. */
+int lise_create(int nx, int ny, int nz, double dx, double dt, int nwf_n, int nwf_p, lise_ctx **out);
+void lise_destroy(lise_ctx *ctx);
+
+int lise_set_params(lise_ctx *ctx, const lise_params *p);
+int lise_set_stream(lise_ctx *ctx, void *cuda_stream);       /* cudaStream_t owned by the caller */
+/* Changes dt and restarts the multistep method (the next 3 steps use the starter). */
+int lise_set_dt(lise_ctx *ctx, double dt);
+/* Number of states processed per kernel launch (L2-resident batching of intermediates); <= 0 restores the default. */
+int lise_set_chunk(lise_ctx *ctx, int nstates);
+
+/* Copies nwf_q states in (device pointer, layout above), accumulates their densities and resets the
+ * multistep history, step counter and time. */
+int lise_set_wavefunctions(lise_ctx *ctx, int species, const void *psi_dev);
+int lise_get_wavefunctions(lise_ctx *ctx, int species, void *psi_dev);
+
+/* Local densities of the current wavefunctions of one species in the layout of the paper's
+ * d_densities (Table 2): 14*Nxyz doubles = n, tau, s(3), div J, j(3), curl j(3),
+ * kappa (re, im).  Eq. 3 with tau via Eq. 51. */
+int lise_densities(lise_ctx *ctx, int species, double *out14_dev);
+/* Mean-field and pairing potentials of one species from the current densities of both species,
+ * rows 0..13 of the paper's d_potentials (Table 3): U, hbar^2/2m*, lap(hbar^2/2m*),
+ * W(3), S(3), A(3), Delta (re, im).  Eqs. 13-21 in the adopted reading. */
+int lise_potentials(lise_ctx *ctx, int species, double *out14_dev);
+
+/* out = H * in for nstates states of `species` (Eq. 11 with mu = 0; h of Eq. 12 in the lattice form
+ * of Eqs. 55, 56), H built from the densities of the context's current wavefunctions of both
+ * species.  No eta subtraction, no 1/(i hbar).  in_dev and out_dev must not overlap. */
+int lise_apply_h(lise_ctx *ctx, int species, const void *in_dev, void *out_dev, int nstates);
+
+/* Advances all states by nsteps time steps: the first 3 steps after lise_set_wavefunctions /
+ * lise_set_dt use the 4th-order series expansion with predictor-corrector densities (Eqs. 75-77),
+ * later steps the ABM predictor-modifier-corrector (Eq. 78 a-d) with 2 H evaluations per step and
+ * the phase removal of Eqs. 80-81. */
+int lise_step(lise_ctx *ctx, int nsteps);
+
+/* Energy, particle numbers, norm / orthonormality defects of the current wavefunctions. Synchronises. */
+int lise_observables(lise_ctx *ctx, lise_observables_t *host_out);
+
+/* Per-kernel-class device timing with CUDA events on the context's stream (for bench.py's roofline).
+ * lise_profile(ctx, 1) starts recording an event pair around every launch of the per-state kernels
+ * (and around each grid-only phase); lise_profile_read synchronises and returns the summed
+ * milliseconds and launch counts per class, then clears the record.  Classes:
+ *   0 H-apply on yz-planes (y and z lines), 1 H-apply on xz-planes (x lines, eta),
+ *   2 ABM update + y/z density pass, 3 x density pass, 4 grid-only phase (reduction, potentials, Coulomb).
+ * ms and counts are HOST arrays of 5 entries. */
+int lise_profile(lise_ctx *ctx, int enable);
+int lise_profile_read(lise_ctx *ctx, double *ms, long *counts);
+
+/* Number of kernel launches issued by this context so far (for bench.py's gpu_launches). */
+long lise_launch_count(const lise_ctx *ctx);
+/* Bytes of device memory held by the context. */
+long long lise_device_bytes(const lise_ctx *ctx);
+
+const char *lise_strerror(int code);
+const char *lise_last_error(const lise_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,755 @@
+// lise.cu -- C-ABI entry points (include/lise.h) and host-side orchestration of the TDSLDA step.
+//
+// Resident state arrays per species ("slots", roles rotate by pointer swap):
+//   A y_n | B y_{n-1} -> Q -> y_{n+1} | C f_{n-3} -> f_n | D f_{n-1} | E f_{n-2} | F e_n -> m -> e_{n+1} | G p
+// One ABM step (Eq. 78) = two evaluations; each evaluation = grid-only potentials, then per
+// chunk of states: k_happly<0> (yz-planes) -> k_happly<1> (xz-planes, eta) -> k_update_yz (ABM + y/z
+// densities of the new state) -> k_dens_x (x densities of the new state).
+#include "common.cuh"
+#include "state_kernels.cuh"
+#include "grid_kernels.cuh"
+#include <new>
+#include <stdlib.h>
+#include <vector>
+
+enum { RA = 0, RB, RC, RD, RE, RF, RG };
+
+struct lise_ctx {
+    Lattice L;
+    int n[3];
+    double dt;
+    int nwf[2];
+    lise_params par;
+    PhysConst pc;
+    cudaStream_t stream;
+    double2* ctab[3];
+    cplx* slot[2][LISE_NSLOT];
+    int role[LISE_NSLOT];
+    cplx* W;
+    int chunk, wcap;
+    double *eta_part, *eta_fix;
+    int G;
+    double *part[2], *acc[2], *acc0[2], *dens[2], *pot[2], *geff[2];
+    double *gtmp, *phi;
+    GJob *jobs1, *jobs2;
+    int njobs1, njobs2;
+    int P; double Dc;
+    cplx *tw, *cA1, *cA2, *cA3;
+    double* ebuf; int eblocks;
+    cplx* ovl;
+    int R, thr[2];
+    size_t smem_h[2], smem_u, smem_d;
+    int have[2], pot_valid;
+    long step; double time;
+    long launches; long long bytes;
+    std::vector<void*>* allocs;
+    // optional per-kernel-class timing with CUDA events on the context's stream (lise_profile)
+    int prof; int prof_n;
+    std::vector<cudaEvent_t>* prof_ev;      // pairs (start, stop)
+    std::vector<int>* prof_cls;
+    char err[256];
+};
+
+enum { PC_HAPPLY_YZ = 0, PC_HAPPLY_XZ, PC_UPDATE, PC_DENS_X, PC_GRID, PC_NCLASS };
+
+static void prof_begin(lise_ctx* c, int cls)
+{
+    if (!c->prof) return;
+    if ((size_t)(2 * c->prof_n + 2) > c->prof_ev->size()) {
+        cudaEvent_t a, b; cudaEventCreate(&a); cudaEventCreate(&b);
+        c->prof_ev->push_back(a); c->prof_ev->push_back(b); c->prof_cls->push_back(cls);
+    }
+    (*c->prof_cls)[c->prof_n] = cls;
+    cudaEventRecord((*c->prof_ev)[2 * c->prof_n], c->stream);
+}
+static void prof_end(lise_ctx* c)
+{
+    if (!c->prof) return;
+    cudaEventRecord((*c->prof_ev)[2 * c->prof_n + 1], c->stream);
+    c->prof_n++;
+}
+
+static const char* g_noctx = "no context";
+
+#define CK(call)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess) {                                                                   \
+            snprintf(c->err, sizeof(c->err), "%s:%d %s: %s", __FILE__, __LINE__, #call, cudaGetErrorString(e_)); \
+            return (e_ == cudaErrorMemoryAllocation) ? LISE_ENOMEM : LISE_ECUDA;                   \
+        }                                                                                          \
+    } while (0)
+#define CKL()                                                                                      \
+    do { c->launches++; CK(cudaGetLastError()); } while (0)
+#define TRY(expr) do { int rc_ = (expr); if (rc_ != LISE_OK) return rc_; } while (0)
+
+static int dmalloc(lise_ctx* c, void** p, size_t bytes)
+{
+    if (bytes == 0) bytes = 16;
+    CK(cudaMalloc(p, bytes));
+    c->allocs->push_back(*p);
+    c->bytes += (long long)bytes;
+    return LISE_OK;
+}
+#define DM(ptr, count) TRY(dmalloc(c, (void**)&(ptr), sizeof(*(ptr)) * (size_t)(count)))
+
+static inline unsigned nblk(size_t n, int t) { return (unsigned)((n + t - 1) / t); }
+static inline cplx* S(lise_ctx* c, int q, int r) { return c->slot[q][c->role[r]]; }
+
+// ---- tables: closed-form DVR coefficients (Eq. 48a; Eq. 48b with prefactor 2 pi^2 / (N a)^2) ----
+static void host_ctab(int N, double a, std::vector<double2>& t)
+{
+    std::vector<double> c1(N), c2(N);
+    const long double pi = 3.14159265358979323846264338327950288L;
+    c1[0] = 0.0;
+    c2[0] = (double)(-pi * pi / (3.0L * a * a) * (1.0L + 2.0L / ((long double)N * N)));
+    for (int k = 1; k < N; ++k) {
+        long double th = pi * k / N;
+        long double sgn = (k % 2) ? -1.0L : 1.0L;
+        c1[k] = (2 * k == N) ? 0.0 : (double)(pi / (N * (long double)a) * sgn * cosl(th) / sinl(th));
+        c2[k] = (double)(-2.0L * pi * pi / ((long double)N * N * a * a) * sgn / (sinl(th) * sinl(th)));
+    }
+    t.resize(2 * N);
+    for (int d = -N; d < N; ++d) {
+        int k = ((d % N) + N) % N;
+        t[N + d] = make_double2(c1[k], c2[k]);
+    }
+}
+
+static void set_physconst(lise_ctx* c)
+{
+    const lise_params& p = c->par;
+    PhysConst& k = c->pc;
+    k.h2m = p.hbar2_2m; k.e2 = p.e2; k.hbarc = p.hbarc; k.gamma = p.gamma; k.a = c->L.dx;
+    k.Kc = 2.442749607806335;
+    // couplings of Eq. 9 from the Skyrme parameters (standard relations, DESIGN.md A.0)
+    k.Cn[0] = 3.0 * p.t0 / 8.0;                       k.Cn[1] = -(p.t0 / 4.0) * (0.5 + p.x0);
+    k.Cg[0] = p.t3 / 16.0;                            k.Cg[1] = -(p.t3 / 24.0) * (0.5 + p.x3);
+    k.Cd[0] = -9.0 * p.t1 / 64.0 + (p.t2 / 16.0) * (1.25 + p.x2);
+    k.Cd[1] = (3.0 * p.t1 / 32.0) * (0.5 + p.x1) + (p.t2 / 32.0) * (0.5 + p.x2);
+    k.Ct[0] = 3.0 * p.t1 / 16.0 + (p.t2 / 4.0) * (1.25 + p.x2);
+    k.Ct[1] = -(p.t1 / 8.0) * (0.5 + p.x1) + (p.t2 / 8.0) * (0.5 + p.x2);
+    k.CJ[0] = -3.0 * p.W0 / 4.0;                      k.CJ[1] = -p.W0 / 4.0;
+    k.g0[0] = p.g0_n; k.g0[1] = p.g0_p;
+    k.coulomb = p.coulomb && c->nwf[1] > 0; k.rearr = p.pairing_rearrangement;
+}
+
+extern "C" int lise_default_params(lise_params* p)
+{
+    if (!p) return LISE_EINVAL;
+    p->hbar2_2m = 20.73553; p->e2 = 1.439964; p->hbarc = 197.3269804;
+    p->t0 = -2488.91; p->t1 = 486.82; p->t2 = -546.39; p->t3 = 13777.0;
+    p->x0 = 0.834; p->x1 = -0.344; p->x2 = -1.000; p->x3 = 1.354;
+    p->gamma = 1.0 / 6.0; p->W0 = 123.0;
+    p->g0_n = -250.0; p->g0_p = -250.0;
+    p->coulomb = 1; p->pairing_rearrangement = 1; p->remove_phase = 1;
+    return LISE_OK;
+}
+
+// ---- kernel launch helpers (dispatch on the register blocking R) ----
+template <int KIND>
+static int launch_happly(lise_ctx* c, const HArgs& a)
+{
+    dim3 grid(KIND == 0 ? c->L.nx : c->L.ny, c->G);
+    const int t = c->thr[KIND]; const size_t sm = c->smem_h[KIND];
+    prof_begin(c, KIND == 0 ? PC_HAPPLY_YZ : PC_HAPPLY_XZ);
+    switch (c->R) {
+    case 8: k_happly<KIND, 8><<<grid, t, sm, c->stream>>>(a); break;
+    case 4: k_happly<KIND, 4><<<grid, t, sm, c->stream>>>(a); break;
+    default: k_happly<KIND, 2><<<grid, t, sm, c->stream>>>(a); break;
+    }
+    prof_end(c);
+    CKL();
+    return LISE_OK;
+}
+template <int MODE>
+static int launch_update(lise_ctx* c, const UArgs& a)
+{
+    dim3 grid(c->L.nx, c->G);
+    const int t = c->thr[0]; const size_t sm = c->smem_u;
+    prof_begin(c, PC_UPDATE);
+    switch (c->R) {
+    case 8: k_update_yz<MODE, 8><<<grid, t, sm, c->stream>>>(a); break;
+    case 4: k_update_yz<MODE, 4><<<grid, t, sm, c->stream>>>(a); break;
+    default: k_update_yz<MODE, 2><<<grid, t, sm, c->stream>>>(a); break;
+    }
+    prof_end(c);
+    CKL();
+    return LISE_OK;
+}
+static int launch_dens_x(lise_ctx* c, const DArgs& a)
+{
+    dim3 grid(c->L.ny, c->G);
+    const int t = c->thr[1]; const size_t sm = c->smem_d;
+    prof_begin(c, PC_DENS_X);
+    switch (c->R) {
+    case 8: k_dens_x<8><<<grid, t, sm, c->stream>>>(a); break;
+    case 4: k_dens_x<4><<<grid, t, sm, c->stream>>>(a); break;
+    default: k_dens_x<2><<<grid, t, sm, c->stream>>>(a); break;
+    }
+    prof_end(c);
+    CKL();
+    return LISE_OK;
+}
+template <typename K>
+static cudaError_t set_smem(K kern, size_t bytes)
+{
+    return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+template <int R>
+static int set_attrs(lise_ctx* c)
+{
+    CK(set_smem(k_happly<0, R>, c->smem_h[0]));
+    CK(set_smem(k_happly<1, R>, c->smem_h[1]));
+    CK(set_smem(k_update_yz<0, R>, c->smem_u));
+    CK(set_smem(k_update_yz<1, R>, c->smem_u));
+    CK(set_smem(k_update_yz<2, R>, c->smem_u));
+    CK(set_smem(k_update_yz<3, R>, c->smem_u));
+    CK(set_smem(k_dens_x<R>, c->smem_d));
+    return LISE_OK;
+}
+
+static void fill_common(lise_ctx* c, const double2** ct) { for (int i = 0; i < 3; ++i) ct[i] = c->ctab[i]; }
+
+// W = H X for ns states (ns <= chunk) of species q
+static int apply_h_chunk(lise_ctx* c, int q, const cplx* X, cplx* W, int ns)
+{
+    HArgs a;
+    a.L = c->L; a.X = X; a.W = W; a.pot = c->pot[q]; fill_common(c, a.ctab);
+    a.eta_part = c->eta_part; a.ns = ns; a.G = c->G;
+    TRY(launch_happly<0>(c, a));
+    TRY(launch_happly<1>(c, a));
+    return LISE_OK;
+}
+
+static UArgs make_uargs(lise_ctx* c, int q, size_t off, int ns)
+{
+    UArgs u;
+    u.L = c->L; u.W = c->W;
+    u.sA = S(c, q, RA) + off; u.sB = S(c, q, RB) + off; u.sC = S(c, q, RC) + off; u.sD = S(c, q, RD) + off;
+    u.sE = S(c, q, RE) + off; u.sF = S(c, q, RF) + off; u.sG = S(c, q, RG) + off;
+    u.Z = nullptr; u.eta_part = c->eta_part; u.eta_fix = c->eta_fix; u.part = c->part[q];
+    fill_common(c, u.ctab);
+    u.dt = c->dt; u.hbarc = c->par.hbarc; u.ns = ns; u.G = c->G; u.order = 0; u.remove_phase = c->par.remove_phase;
+    u.write_f = 1;
+    return u;
+}
+
+static int zero_partials(lise_ctx* c, int q)
+{
+    CK(cudaMemsetAsync(c->part[q], 0, sizeof(double) * (size_t)c->G * LISE_NACC * c->L.nxyz, c->stream));
+    return LISE_OK;
+}
+
+// part[q] += densities of the nwf[q] states in Z (both passes)
+static int dens_accumulate(lise_ctx* c, int q, const cplx* Z)
+{
+    const size_t slen = (size_t)4 * c->L.nxyz;
+    for (int s0 = 0; s0 < c->nwf[q]; s0 += c->chunk) {
+        const int ns = (c->nwf[q] - s0 < c->chunk) ? c->nwf[q] - s0 : c->chunk;
+        UArgs u = make_uargs(c, q, 0, ns);
+        u.Z = Z + s0 * slen;
+        TRY(launch_update<0>(c, u));
+        DArgs d; d.L = c->L; d.Z = Z + s0 * slen; d.part = c->part[q]; fill_common(c, d.ctab); d.ns = ns; d.G = c->G;
+        TRY(launch_dens_x(c, d));
+    }
+    return LISE_OK;
+}
+
+static int reduce_partials(lise_ctx* c, int q)
+{
+    const size_t n = (size_t)LISE_NACC * c->L.nxyz;
+    k_reduce_partials<<<nblk(n, 256), 256, 0, c->stream>>>(c->part[q], c->G, n, c->acc[q]);
+    CKL();
+    return LISE_OK;
+}
+
+static int coulomb(lise_ctx* c, const double* np)
+{
+    const int nx = c->L.nx, ny = c->L.ny, nz = c->L.nz, P = c->P;
+    const int T = 128;
+    k_dft_pass_real<<<nblk((size_t)nx * ny * P, T), T, 0, c->stream>>>(np, c->cA1, c->tw, nx * ny, nz, P, 1, P); CKL();
+    k_dft_pass<1><<<nblk((size_t)nx * P * P, T), T, 0, c->stream>>>(c->cA1, c->cA2, c->tw, nx, ny, P, P, P); CKL();
+    k_dft_pass<1><<<nblk((size_t)P * P * P, T), T, 0, c->stream>>>(c->cA2, c->cA3, c->tw, 1, nx, P, P * P, P); CKL();
+    k_coulomb_kernel_mult<<<nblk((size_t)P * P * P, 256), 256, 0, c->stream>>>(c->cA3, P, c->L.dx, c->Dc); CKL();
+    k_dft_pass<-1><<<nblk((size_t)nx * P * P, T), T, 0, c->stream>>>(c->cA3, c->cA2, c->tw, 1, P, nx, P * P, P); CKL();
+    k_dft_pass<-1><<<nblk((size_t)nx * ny * P, T), T, 0, c->stream>>>(c->cA2, c->cA1, c->tw, nx, P, ny, P, P); CKL();
+    const double scale = c->par.e2 / ((double)P * P * P);
+    k_dft_pass_final<<<nblk((size_t)nx * ny * nz, T), T, 0, c->stream>>>(c->cA1, c->phi, c->tw, nx * ny, P, nz, P, scale); CKL();
+    return LISE_OK;
+}
+
+// potentials of both species from the reduced accumulators acc[0], acc[1]
+static int compute_potentials(lise_ctx* c)
+{
+    const int nx = c->L.nxyz;
+    if (c->pc.coulomb) TRY(coulomb(c, c->acc[1] + (size_t)ACC_N * nx));
+    k_grid_deriv<<<dim3(nblk(nx, 128), c->njobs1), 128, 0, c->stream>>>(c->L, c->jobs1, c->ctab[0], c->ctab[1], c->ctab[2]); CKL();
+    k_potentials<<<nblk(nx, 128), 128, 0, c->stream>>>(c->L, c->pc, c->acc[0], c->acc[1], c->gtmp, c->phi,
+                                                        c->dens[0], c->dens[1], c->pot[0], c->pot[1], c->geff[0], c->geff[1]); CKL();
+    k_grid_deriv<<<dim3(nblk(nx, 128), c->njobs2), 128, 0, c->stream>>>(c->L, c->jobs2, c->ctab[0], c->ctab[1], c->ctab[2]); CKL();
+    k_uloc<<<nblk(nx, 128), 128, 0, c->stream>>>(nx, c->pot[0], c->pot[1]); CKL();
+    return LISE_OK;
+}
+
+// grid-only work between the barriers, timed as one class
+static int grid_phase(lise_ctx* c, int reduce)
+{
+    prof_begin(c, PC_GRID);
+    if (reduce) { TRY(reduce_partials(c, 0)); TRY(reduce_partials(c, 1)); }
+    TRY(compute_potentials(c));
+    prof_end(c);
+    return LISE_OK;
+}
+
+static int ensure_potentials(lise_ctx* c)
+{
+    if (c->pot_valid) return LISE_OK;
+    TRY(grid_phase(c, 1));
+    c->pot_valid = 1;
+    return LISE_OK;
+}
+
+static void rotate_f(lise_ctx* c)
+{
+    const int rc = c->role[RC], rd = c->role[RD], re = c->role[RE];
+    c->role[RD] = rc; c->role[RE] = rd; c->role[RC] = re;
+}
+
+// one ABM predictor-modifier-corrector step (Eq. 78)
+static int abm_step(lise_ctx* c)
+{
+    const size_t slen = (size_t)4 * c->L.nxyz;
+    TRY(ensure_potentials(c));                      // potentials of y_n
+    for (int phase = 1; phase <= 2; ++phase) {
+        TRY(zero_partials(c, 0)); TRY(zero_partials(c, 1));
+        for (int q = 0; q < 2; ++q)
+            for (int s0 = 0; s0 < c->nwf[q]; s0 += c->chunk) {
+                const int ns = (c->nwf[q] - s0 < c->chunk) ? c->nwf[q] - s0 : c->chunk;
+                const size_t off = s0 * slen;
+                const cplx* X = (phase == 1 ? S(c, q, RA) : S(c, q, RF)) + off;
+                TRY(apply_h_chunk(c, q, X, c->W, ns));
+                UArgs u = make_uargs(c, q, off, ns);
+                if (phase == 1) TRY(launch_update<1>(c, u)); else TRY(launch_update<2>(c, u));
+                DArgs d; d.L = c->L; d.Z = (phase == 1 ? S(c, q, RF) : S(c, q, RB)) + off; d.part = c->part[q];
+                fill_common(c, d.ctab); d.ns = ns; d.G = c->G;
+                TRY(launch_dens_x(c, d));
+            }
+        if (phase == 1) TRY(grid_phase(c, 1));     // potentials of the modifier m
+    }
+    // y_{n+1} sits in B: A <-> B; f history shifts
+    const int ra = c->role[RA]; c->role[RA] = c->role[RB]; c->role[RB] = ra;
+    rotate_f(c);
+    c->pot_valid = 0;                               // part[] now holds the densities of y_{n+1}
+    return LISE_OK;
+}
+
+// T4(P) applied to y_n of every state: acc (slot F) = sum_{m<=4} (1/m!) [dt (H - eta)/(i hbar c)]^m y_n  (Eq. 77)
+static int taylor4_all(lise_ctx* c, int write_f)
+{
+    const size_t slen = (size_t)4 * c->L.nxyz;
+    for (int q = 0; q < 2; ++q)
+        for (int s0 = 0; s0 < c->nwf[q]; s0 += c->chunk) {
+            const int ns = (c->nwf[q] - s0 < c->chunk) ? c->nwf[q] - s0 : c->chunk;
+            const size_t off = s0 * slen;
+            for (int m = 1; m <= 4; ++m) {
+                const cplx* X = (m == 1 ? S(c, q, RA) : S(c, q, RG)) + off;
+                TRY(apply_h_chunk(c, q, X, c->W, ns));
+                UArgs u = make_uargs(c, q, off, ns);
+                u.order = m; u.write_f = write_f;
+                TRY(launch_update<3>(c, u));
+            }
+        }
+    return LISE_OK;
+}
+
+// one start-up step: series expansion with predictor-corrector densities (Eqs. 75-77)
+static int starter_step(lise_ctx* c)
+{
+    const size_t nacc = (size_t)LISE_NACC * c->L.nxyz;
+    TRY(ensure_potentials(c));                      // H(t) from n(t); acc[] = accumulators of y_n
+    for (int q = 0; q < 2; ++q)
+        CK(cudaMemcpyAsync(c->acc0[q], c->acc[q], sizeof(double) * nacc, cudaMemcpyDeviceToDevice, c->stream));
+    TRY(taylor4_all(c, 1));                         // psi_pre -> F, f_n -> C
+    for (int q = 0; q < 2; ++q) {                   // n_cor = (n_pre + n(t)) / 2
+        TRY(zero_partials(c, q));
+        TRY(dens_accumulate(c, q, S(c, q, RF)));
+        TRY(reduce_partials(c, q));
+        k_average<<<nblk(nacc, 256), 256, 0, c->stream>>>(c->acc[q], c->acc0[q], nacc); CKL();
+    }
+    TRY(compute_potentials(c));                     // H_cor
+    TRY(taylor4_all(c, 0));                         // y_{n+1} -> F
+    for (int q = 0; q < 2; ++q) {
+        TRY(zero_partials(c, q));
+        TRY(dens_accumulate(c, q, S(c, q, RF)));
+    }
+    // A' = F (y_{n+1}), B' = A (y_n), F' = old B cleared (e = 0); f history shifts
+    const int ra = c->role[RA], rb = c->role[RB], rf = c->role[RF];
+    c->role[RA] = rf; c->role[RB] = ra; c->role[RF] = rb;
+    rotate_f(c);
+    for (int q = 0; q < 2; ++q)
+        CK(cudaMemsetAsync(S(c, q, RF), 0, sizeof(cplx) * (size_t)c->nwf[q] * 4 * c->L.nxyz, c->stream));
+    c->pot_valid = 0;
+    return LISE_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// C ABI
+// ------------------------------------------------------------------------------------------------
+static int build_jobs(lise_ctx* c)
+{
+    const size_t nx = c->L.nxyz;
+    std::vector<GJob> j1, j2;
+    auto term = [](const double* in, int axis, int order, double sign) { GTerm t; t.in = in; t.axis = axis; t.order = order; t.sign = sign; return t; };
+    for (int q = 0; q < 2; ++q) {
+        const double* a = c->acc[q];
+        double* g = c->gtmp + (size_t)q * GT_PER_Q * nx;
+        GJob jb;
+        // lap n
+        jb.nterms = 3; jb.out = g + (size_t)GT_LAPN * nx;
+        for (int i = 0; i < 3; ++i) jb.t[i] = term(a + (size_t)ACC_N * nx, i, 2, 1.0);
+        j1.push_back(jb);
+        // grad n
+        for (int i = 0; i < 3; ++i) { jb.nterms = 1; jb.out = g + (size_t)(GT_GRADN + i) * nx; jb.t[0] = term(a + (size_t)ACC_N * nx, i, 1, 1.0); j1.push_back(jb); }
+        // div J
+        jb.nterms = 3; jb.out = g + (size_t)GT_DIVJ * nx;
+        for (int i = 0; i < 3; ++i) jb.t[i] = term(a + (size_t)(ACC_J + i) * nx, i, 1, 1.0);
+        j1.push_back(jb);
+        // curl j, curl s: (curl v)_k = D_i v_j - D_j v_i, (k, i, j) cyclic
+        for (int w = 0; w < 2; ++w) {
+            const int src = w ? ACC_S : ACC_JC, dst = w ? GT_CURLS : GT_CURLJ;
+            for (int k = 0; k < 3; ++k) {
+                const int i = (k + 1) % 3, jx = (k + 2) % 3;
+                jb.nterms = 2; jb.out = g + (size_t)(dst + k) * nx;
+                jb.t[0] = term(a + (size_t)(src + jx) * nx, i, 1, 1.0);
+                jb.t[1] = term(a + (size_t)(src + i) * nx, jx, 1, -1.0);
+                j1.push_back(jb);
+            }
+        }
+        // lap M
+        jb.nterms = 3; jb.out = c->pot[q] + (size_t)P_LAPM * nx;
+        for (int i = 0; i < 3; ++i) jb.t[i] = term(c->pot[q] + (size_t)P_M * nx, i, 2, 1.0);
+        j2.push_back(jb);
+    }
+    c->njobs1 = (int)j1.size(); c->njobs2 = (int)j2.size();
+    DM(c->jobs1, j1.size()); DM(c->jobs2, j2.size());
+    CK(cudaMemcpy(c->jobs1, j1.data(), sizeof(GJob) * j1.size(), cudaMemcpyHostToDevice));
+    CK(cudaMemcpy(c->jobs2, j2.data(), sizeof(GJob) * j2.size(), cudaMemcpyHostToDevice));
+    return LISE_OK;
+}
+
+static int default_chunk(const lise_ctx* c)
+{
+    const double sbytes = 64.0 * c->L.nxyz;
+    int nmax = c->nwf[0] > c->nwf[1] ? c->nwf[0] : c->nwf[1];
+    int ch = (int)(32.0 * 1048576.0 / sbytes);
+    if (ch < c->G) ch = c->G;
+    ch = (ch / c->G) * c->G;
+    if (ch > nmax) ch = nmax;
+    if (ch < 1) ch = 1;
+    return ch;
+}
+
+static int ctx_init(lise_ctx* c)
+{
+    const Lattice& L = c->L;
+    const size_t nx = L.nxyz;
+    // blocking and launch shapes
+    c->R = (L.nx % 4 == 0 && L.ny % 4 == 0 && L.nz % 4 == 0) ? 4 : 2;
+    if (const char* e = getenv("LISE_R")) {
+        int r = atoi(e);
+        if ((r == 2 || r == 4 || r == 8) && L.nx % r == 0 && L.ny % r == 0 && L.nz % r == 0) c->R = r;
+    }
+    const int ld = L.nz + 1;
+    const int n1[2] = {L.ny, L.nx};
+    for (int k = 0; k < 2; ++k) {
+        const int npts = n1[k] * L.nz;
+        int t = ((2 * npts / c->R + 31) / 32) * 32;
+        if (t > 512) t = 512;
+        if (t < 64) t = 64;
+        c->thr[k] = t;
+        c->smem_h[k] = sizeof(double2) * (size_t)(2 * (n1[k] + L.nz) + 8 * n1[k] * ld) + 64 * sizeof(double);
+    }
+    c->smem_u = sizeof(double2) * (size_t)(2 * (L.ny + L.nz) + 6 * L.ny * ld) + 64 * sizeof(double);
+    c->smem_d = sizeof(double2) * (size_t)(2 * L.nx + 6 * L.nx * ld);
+    const size_t lim = 227 * 1024;
+    if (c->smem_h[0] > lim || c->smem_h[1] > lim || c->smem_u > lim || c->smem_d > lim) {
+        snprintf(c->err, sizeof(c->err), "lattice planes too large for shared memory (%zu bytes needed, %zu available)",
+                 c->smem_h[0] > c->smem_h[1] ? c->smem_h[0] : c->smem_h[1], lim);
+        return LISE_EUNSUPPORTED;
+    }
+    if (c->R == 8) TRY(set_attrs<8>(c)); else if (c->R == 4) TRY(set_attrs<4>(c)); else TRY(set_attrs<2>(c));
+    int minp = L.nx < L.ny ? L.nx : L.ny;
+    c->G = (2 * 148 + minp - 1) / minp;
+    if (c->G > LISE_MAXG) c->G = LISE_MAXG;
+    if (c->G < 1) c->G = 1;
+    c->chunk = default_chunk(c);
+    const int nmax = c->nwf[0] > c->nwf[1] ? c->nwf[0] : c->nwf[1];
+
+    // derivative tables
+    for (int i = 0; i < 3; ++i) {
+        std::vector<double2> t;
+        host_ctab(c->n[i], L.dx, t);
+        DM(c->ctab[i], t.size());
+        CK(cudaMemcpy(c->ctab[i], t.data(), sizeof(double2) * t.size(), cudaMemcpyHostToDevice));
+    }
+    // state slots and scratch
+    for (int q = 0; q < 2; ++q)
+        for (int s = 0; s < LISE_NSLOT; ++s) {
+            DM(c->slot[q][s], (size_t)c->nwf[q] * 4 * nx);
+            CK(cudaMemset(c->slot[q][s], 0, sizeof(cplx) * (size_t)c->nwf[q] * 4 * nx));
+        }
+    for (int s = 0; s < LISE_NSLOT; ++s) c->role[s] = s;
+    c->wcap = nmax < 512 ? (nmax > 0 ? nmax : 1) : 512;     // largest chunk lise_set_chunk accepts
+    if (c->wcap < c->chunk) c->wcap = c->chunk;
+    DM(c->W, (size_t)c->wcap * 4 * nx);
+    DM(c->eta_part, (size_t)c->wcap * L.ny);
+    DM(c->eta_fix, (size_t)c->wcap);
+    for (int q = 0; q < 2; ++q) {
+        DM(c->part[q], (size_t)LISE_MAXG * LISE_NACC * nx);
+        CK(cudaMemset(c->part[q], 0, sizeof(double) * (size_t)LISE_MAXG * LISE_NACC * nx));
+        DM(c->acc[q], LISE_NACC * nx); DM(c->acc0[q], LISE_NACC * nx);
+        DM(c->dens[q], 14 * nx); DM(c->pot[q], LISE_NPOT * nx); DM(c->geff[q], nx);
+        CK(cudaMemset(c->pot[q], 0, sizeof(double) * LISE_NPOT * nx));
+    }
+    DM(c->gtmp, 2 * GT_PER_Q * nx);
+    DM(c->phi, nx);
+    CK(cudaMemset(c->phi, 0, sizeof(double) * nx));
+    TRY(build_jobs(c));
+    // Coulomb
+    int nm = L.nx; if (L.ny > nm) nm = L.ny; if (L.nz > nm) nm = L.nz;
+    c->P = 3 * nm; c->Dc = sqrt(3.0) * L.dx * nm;
+    if (c->nwf[1] > 0) {
+        const int P = c->P;
+        std::vector<double2> tw(P);
+        const long double pi = 3.14159265358979323846264338327950288L;
+        for (int r = 0; r < P; ++r) { long double ph = 2.0L * pi * r / P; tw[r] = make_double2((double)cosl(ph), (double)-sinl(ph)); }
+        DM(c->tw, P);
+        CK(cudaMemcpy(c->tw, tw.data(), sizeof(double2) * P, cudaMemcpyHostToDevice));
+        DM(c->cA1, (size_t)L.nx * L.ny * P); DM(c->cA2, (size_t)L.nx * P * P); DM(c->cA3, (size_t)P * P * P);
+    }
+    c->eblocks = 64;
+    DM(c->ebuf, c->eblocks * 6);
+    DM(c->ovl, (size_t)(nmax > 0 ? nmax : 1) * 4);
+    return LISE_OK;
+}
+
+extern "C" int lise_create(int nx, int ny, int nz, double dx, double dt, int nwf_n, int nwf_p, lise_ctx** out)
+{
+    if (!out) return LISE_EINVAL;
+    *out = nullptr;
+    if (nx < 2 || ny < 2 || nz < 2 || ((nx | ny | nz) & 1) || !(dx > 0.0) || nwf_n < 0 || nwf_p < 0) return LISE_EINVAL;
+    if ((long long)nx * ny * nz > (1LL << 26)) return LISE_EUNSUPPORTED;
+    lise_ctx* c = new (std::nothrow) lise_ctx();
+    if (!c) return LISE_ENOMEM;
+    memset(c, 0, sizeof(*c));
+    c->allocs = new std::vector<void*>();
+    c->prof_ev = new std::vector<cudaEvent_t>();
+    c->prof_cls = new std::vector<int>();
+    c->L.nx = nx; c->L.ny = ny; c->L.nz = nz; c->L.nxyz = nx * ny * nz; c->L.dx = dx; c->L.dV = dx * dx * dx;
+    c->n[0] = nx; c->n[1] = ny; c->n[2] = nz;
+    c->dt = dt; c->nwf[0] = nwf_n; c->nwf[1] = nwf_p;
+    lise_default_params(&c->par);
+    if (nwf_p == 0) c->par.coulomb = 0;
+    set_physconst(c);
+    c->stream = 0;
+    c->have[0] = (nwf_n == 0); c->have[1] = (nwf_p == 0);
+    int rc = ctx_init(c);
+    if (rc != LISE_OK) {
+        fprintf(stderr, "lise_create: %s\n", c->err);
+        lise_destroy(c);
+        return rc;
+    }
+    *out = c;
+    return LISE_OK;
+}
+
+extern "C" void lise_destroy(lise_ctx* c)
+{
+    if (!c) return;
+    cudaStreamSynchronize(c->stream);
+    if (c->allocs) {
+        for (void* p : *c->allocs) cudaFree(p);
+        delete c->allocs;
+    }
+    if (c->prof_ev) { for (cudaEvent_t e : *c->prof_ev) cudaEventDestroy(e); delete c->prof_ev; }
+    delete c->prof_cls;
+    delete c;
+}
+
+extern "C" int lise_set_params(lise_ctx* c, const lise_params* p)
+{
+    if (!c || !p) return LISE_EINVAL;
+    c->par = *p;
+    set_physconst(c);
+    c->pot_valid = 0;
+    return LISE_OK;
+}
+
+extern "C" int lise_set_stream(lise_ctx* c, void* s)
+{
+    if (!c) return LISE_EINVAL;
+    c->stream = (cudaStream_t)s;
+    return LISE_OK;
+}
+
+extern "C" int lise_set_dt(lise_ctx* c, double dt)
+{
+    if (!c) return LISE_EINVAL;
+    c->dt = dt; c->step = 0;
+    return LISE_OK;
+}
+
+extern "C" int lise_set_chunk(lise_ctx* c, int n)
+{
+    if (!c) return LISE_EINVAL;
+    if (n <= 0) c->chunk = default_chunk(c);
+    else c->chunk = n > c->wcap ? c->wcap : n;
+    return LISE_OK;
+}
+
+extern "C" int lise_set_wavefunctions(lise_ctx* c, int q, const void* psi_dev)
+{
+    if (!c || q < 0 || q > 1 || (!psi_dev && c->nwf[q] > 0)) return LISE_EINVAL;
+    const size_t bytes = sizeof(cplx) * (size_t)c->nwf[q] * 4 * c->L.nxyz;
+    if (c->nwf[q] > 0) CK(cudaMemcpyAsync(S(c, q, RA), psi_dev, bytes, cudaMemcpyDeviceToDevice, c->stream));
+    TRY(zero_partials(c, q));
+    if (c->nwf[q] > 0) TRY(dens_accumulate(c, q, S(c, q, RA)));
+    c->have[q] = 1; c->pot_valid = 0; c->step = 0; c->time = 0.0;
+    return LISE_OK;
+}
+
+extern "C" int lise_get_wavefunctions(lise_ctx* c, int q, void* psi_dev)
+{
+    if (!c || q < 0 || q > 1 || (!psi_dev && c->nwf[q] > 0)) return LISE_EINVAL;
+    if (!c->have[q]) { snprintf(c->err, sizeof(c->err), "wavefunctions of species %d not set", q); return LISE_ESTATE; }
+    const size_t bytes = sizeof(cplx) * (size_t)c->nwf[q] * 4 * c->L.nxyz;
+    if (c->nwf[q] > 0) CK(cudaMemcpyAsync(psi_dev, S(c, q, RA), bytes, cudaMemcpyDeviceToDevice, c->stream));
+    return LISE_OK;
+}
+
+static int need_both(lise_ctx* c)
+{
+    if (!c->have[0] || !c->have[1]) { snprintf(c->err, sizeof(c->err), "set the wavefunctions of both species first"); return LISE_ESTATE; }
+    return LISE_OK;
+}
+
+extern "C" int lise_densities(lise_ctx* c, int q, double* out14_dev)
+{
+    if (!c || q < 0 || q > 1 || !out14_dev) return LISE_EINVAL;
+    TRY(need_both(c));
+    TRY(ensure_potentials(c));
+    CK(cudaMemcpyAsync(out14_dev, c->dens[q], sizeof(double) * 14 * (size_t)c->L.nxyz, cudaMemcpyDeviceToDevice, c->stream));
+    return LISE_OK;
+}
+
+extern "C" int lise_potentials(lise_ctx* c, int q, double* out14_dev)
+{
+    if (!c || q < 0 || q > 1 || !out14_dev) return LISE_EINVAL;
+    TRY(need_both(c));
+    TRY(ensure_potentials(c));
+    CK(cudaMemcpyAsync(out14_dev, c->pot[q], sizeof(double) * 14 * (size_t)c->L.nxyz, cudaMemcpyDeviceToDevice, c->stream));
+    return LISE_OK;
+}
+
+extern "C" int lise_apply_h(lise_ctx* c, int q, const void* in_dev, void* out_dev, int nstates)
+{
+    if (!c || q < 0 || q > 1 || !in_dev || !out_dev || nstates < 0) return LISE_EINVAL;
+    TRY(need_both(c));
+    TRY(ensure_potentials(c));
+    const size_t slen = (size_t)4 * c->L.nxyz;
+    const int ch = c->chunk;                       // eta_part scratch is sized for wcap >= chunk states
+    for (int s0 = 0; s0 < nstates; s0 += ch) {
+        const int ns = (nstates - s0 < ch) ? nstates - s0 : ch;
+        TRY(apply_h_chunk(c, q, (const cplx*)in_dev + s0 * slen, (cplx*)out_dev + s0 * slen, ns));
+    }
+    return LISE_OK;
+}
+
+extern "C" int lise_step(lise_ctx* c, int nsteps)
+{
+    if (!c || nsteps < 0) return LISE_EINVAL;
+    TRY(need_both(c));
+    for (int s = 0; s < nsteps; ++s) {
+        if (c->step < 3) TRY(starter_step(c)); else TRY(abm_step(c));
+        c->step += 1; c->time += c->dt;
+    }
+    return LISE_OK;
+}
+
+extern "C" int lise_observables(lise_ctx* c, lise_observables_t* o)
+{
+    if (!c || !o) return LISE_EINVAL;
+    TRY(need_both(c));
+    TRY(ensure_potentials(c));
+    k_energy<<<c->eblocks, 256, 0, c->stream>>>(c->L, c->pc, c->dens[0], c->dens[1], c->gtmp, c->phi, c->geff[0], c->geff[1], c->ebuf); CKL();
+    std::vector<double> eb(c->eblocks * 6);
+    CK(cudaMemcpyAsync(eb.data(), c->ebuf, sizeof(double) * eb.size(), cudaMemcpyDeviceToHost, c->stream));
+    double nd = 0.0, od = 0.0;
+    for (int q = 0; q < 2; ++q) {
+        const int nw = c->nwf[q];
+        if (nw == 0) continue;
+        k_overlaps<<<dim3(nw, 4), 256, 0, c->stream>>>(S(c, q, RA), nw, 4 * c->L.nxyz, c->L.dV, c->ovl); CKL();
+        std::vector<double2> ov((size_t)nw * 4);
+        CK(cudaMemcpyAsync(ov.data(), c->ovl, sizeof(double2) * ov.size(), cudaMemcpyDeviceToHost, c->stream));
+        CK(cudaStreamSynchronize(c->stream));
+        const int ds[4] = {0, 1, 2, nw / 2};
+        for (int k = 0; k < nw; ++k) {
+            const double dn = fabs(ov[(size_t)k * 4].x - 1.0);
+            if (dn > nd) nd = dn;
+            for (int t = 1; t < 4; ++t) {
+                if ((k + ds[t]) % nw == k) continue;
+                const double m = hypot(ov[(size_t)k * 4 + t].x, ov[(size_t)k * 4 + t].y);
+                if (m > od) od = m;
+            }
+        }
+    }
+    CK(cudaStreamSynchronize(c->stream));
+    double e[6] = {0, 0, 0, 0, 0, 0};
+    for (int b = 0; b < c->eblocks; ++b) for (int k = 0; k < 6; ++k) e[k] += eb[b * 6 + k];
+    o->e_kin = e[0]; o->e_skyrme = e[1]; o->e_coul = e[2]; o->e_pair = e[3];
+    o->energy = e[0] + e[1] + e[2] + e[3];
+    o->n_neutron = e[4]; o->n_proton = e[5];
+    o->norm_defect = nd; o->ortho_defect = od;
+    o->time = c->time; o->step = c->step;
+    return LISE_OK;
+}
+
+extern "C" int lise_profile(lise_ctx* c, int enable)
+{
+    if (!c) return LISE_EINVAL;
+    CK(cudaStreamSynchronize(c->stream));
+    c->prof = enable ? 1 : 0; c->prof_n = 0;
+    return LISE_OK;
+}
+
+extern "C" int lise_profile_read(lise_ctx* c, double* ms, long* counts)
+{
+    if (!c || !ms || !counts) return LISE_EINVAL;
+    CK(cudaStreamSynchronize(c->stream));
+    for (int k = 0; k < PC_NCLASS; ++k) { ms[k] = 0.0; counts[k] = 0; }
+    for (int i = 0; i < c->prof_n; ++i) {
+        float t = 0.f;
+        CK(cudaEventElapsedTime(&t, (*c->prof_ev)[2 * i], (*c->prof_ev)[2 * i + 1]));
+        ms[(*c->prof_cls)[i]] += t; counts[(*c->prof_cls)[i]] += 1;
+    }
+    c->prof_n = 0;
+    return LISE_OK;
+}
+
+extern "C" long lise_launch_count(const lise_ctx* c) { return c ? c->launches : 0; }
+extern "C" long long lise_device_bytes(const lise_ctx* c) { return c ? c->bytes : 0; }
+
+extern "C" const char* lise_strerror(int code)
+{
+    switch (code) {
+    case LISE_OK: return "ok";
+    case LISE_EINVAL: return "invalid argument";
+    case LISE_ESTATE: return "wavefunctions not set";
+    case LISE_ECUDA: return "CUDA error";
+    case LISE_ENOMEM: return "out of device memory";
+    case LISE_EUNSUPPORTED: return "unsupported lattice size";
+    default: return "unknown error";
+    }
+}
+extern "C" const char* lise_last_error(const lise_ctx* c) { return c ? c->err : g_noctx; }

@@ -1,0 +1,198 @@
+"""Thin ctypes binding of liblise.so (include/lise.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of the library; torch is used for device memory and
+streams.  There is no CPU fallback: if the library is missing or no CUDA device is present, calls fail.
+"""
+import ctypes as C
+import os
+
+import torch
+
+from . import build as _build
+
+_lib = None
+
+
+class Params(C.Structure):
+    _fields_ = [(n, C.c_double) for n in
+                ("hbar2_2m", "e2", "hbarc", "t0", "t1", "t2", "t3", "x0", "x1", "x2", "x3", "gamma", "W0",
+                 "g0_n", "g0_p")] + [(n, C.c_int) for n in ("coulomb", "pairing_rearrangement", "remove_phase")]
+
+
+class Observables(C.Structure):
+    _fields_ = [(n, C.c_double) for n in
+                ("energy", "e_kin", "e_skyrme", "e_coul", "e_pair", "n_neutron", "n_proton",
+                 "norm_defect", "ortho_defect", "time")] + [("step", C.c_long)]
+
+    def as_dict(self):
+        return {n: getattr(self, n) for n, _ in self._fields_}
+
+
+EXPORTS = ["lise_default_params", "lise_create", "lise_destroy", "lise_set_params", "lise_set_stream",
+           "lise_set_dt", "lise_set_chunk", "lise_set_wavefunctions", "lise_get_wavefunctions",
+           "lise_densities", "lise_potentials", "lise_apply_h", "lise_step", "lise_observables",
+           "lise_profile", "lise_profile_read", "lise_launch_count", "lise_device_bytes", "lise_strerror", "lise_last_error"]
+
+
+def lib_path():
+    return _build.SO
+
+
+def load():
+    """dlopen the in-tree liblise.so (building it with nvcc if the sources are newer)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    try:
+        _build.build()
+    except Exception as exc:  # nvcc missing on the box: use the shipped .so if there is one
+        if not os.path.exists(_build.SO):
+            raise RuntimeError(f"liblise.so is missing and could not be built: {exc}") from exc
+    lib = C.CDLL(_build.SO)
+    vp, ip, dp = C.c_void_p, C.c_int, C.c_double
+    lib.lise_default_params.argtypes = [C.POINTER(Params)]
+    lib.lise_create.argtypes = [ip, ip, ip, dp, dp, ip, ip, C.POINTER(vp)]
+    lib.lise_destroy.argtypes = [vp]; lib.lise_destroy.restype = None
+    lib.lise_set_params.argtypes = [vp, C.POINTER(Params)]
+    lib.lise_set_stream.argtypes = [vp, vp]
+    lib.lise_set_dt.argtypes = [vp, dp]
+    lib.lise_set_chunk.argtypes = [vp, ip]
+    lib.lise_set_wavefunctions.argtypes = [vp, ip, vp]
+    lib.lise_get_wavefunctions.argtypes = [vp, ip, vp]
+    lib.lise_densities.argtypes = [vp, ip, vp]
+    lib.lise_potentials.argtypes = [vp, ip, vp]
+    lib.lise_apply_h.argtypes = [vp, ip, vp, vp, ip]
+    lib.lise_step.argtypes = [vp, ip]
+    lib.lise_observables.argtypes = [vp, C.POINTER(Observables)]
+    lib.lise_profile.argtypes = [vp, ip]
+    lib.lise_profile_read.argtypes = [vp, C.POINTER(dp), C.POINTER(C.c_long)]
+    lib.lise_launch_count.argtypes = [vp]; lib.lise_launch_count.restype = C.c_long
+    lib.lise_device_bytes.argtypes = [vp]; lib.lise_device_bytes.restype = C.c_longlong
+    lib.lise_strerror.argtypes = [ip]; lib.lise_strerror.restype = C.c_char_p
+    lib.lise_last_error.argtypes = [vp]; lib.lise_last_error.restype = C.c_char_p
+    _lib = lib
+    return lib
+
+
+def default_params():
+    p = Params()
+    load().lise_default_params(C.byref(p))
+    return p
+
+
+class LiseError(RuntimeError):
+    pass
+
+
+class Lise:
+    """One TDSLDA context on the current CUDA device.  Tensors are torch CUDA tensors (complex128 / float64)."""
+
+    def __init__(self, nx, ny, nz, dx, dt, nwf_n, nwf_p, params=None, stream=None, device=None):
+        if not torch.cuda.is_available():
+            raise LiseError("no CUDA device: the TDSLDA path has no CPU fallback")
+        self.lib = load()
+        self.device = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
+        self.shape = (nx, ny, nz)
+        self.nxyz = nx * ny * nz
+        self.nwf = (nwf_n, nwf_p)
+        self.dx, self.dt = dx, dt
+        self._h = C.c_void_p()
+        with torch.cuda.device(self.device):
+            rc = self.lib.lise_create(nx, ny, nz, dx, dt, nwf_n, nwf_p, C.byref(self._h))
+        if rc != 0:
+            self._h = C.c_void_p()
+            raise LiseError(f"lise_create failed: {self.lib.lise_strerror(rc).decode()} ({rc})")
+        st = torch.cuda.current_stream(self.device) if stream is None else stream
+        self._chk(self.lib.lise_set_stream(self._h, C.c_void_p(st.cuda_stream)), "lise_set_stream")
+        if params is not None:
+            self.set_params(params)
+
+    def _chk(self, rc, what):
+        if rc != 0:
+            msg = self.lib.lise_last_error(self._h).decode() if self._h else ""
+            raise LiseError(f"{what} failed: {self.lib.lise_strerror(rc).decode()} ({rc}) {msg}")
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self.lib.lise_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _dev(self, t, dtype, numel):
+        if not (t.is_cuda and t.dtype == dtype and t.is_contiguous() and t.numel() == numel):
+            raise LiseError(f"expected a contiguous CUDA {dtype} tensor with {numel} elements, got "
+                            f"{t.dtype} {tuple(t.shape)} on {t.device}")
+        return C.c_void_p(t.data_ptr())
+
+    def set_params(self, params):
+        self._chk(self.lib.lise_set_params(self._h, C.byref(params)), "lise_set_params")
+
+    def set_stream(self, stream):
+        self._chk(self.lib.lise_set_stream(self._h, C.c_void_p(stream.cuda_stream)), "lise_set_stream")
+
+    def set_dt(self, dt):
+        self.dt = dt
+        self._chk(self.lib.lise_set_dt(self._h, dt), "lise_set_dt")
+
+    def set_chunk(self, n):
+        self._chk(self.lib.lise_set_chunk(self._h, n), "lise_set_chunk")
+
+    def set_wavefunctions(self, q, psi):
+        p = self._dev(psi, torch.complex128, self.nwf[q] * 4 * self.nxyz) if self.nwf[q] else C.c_void_p()
+        self._chk(self.lib.lise_set_wavefunctions(self._h, q, p), "lise_set_wavefunctions")
+
+    def get_wavefunctions(self, q, out=None):
+        if out is None:
+            out = torch.empty((self.nwf[q], 4) + self.shape, dtype=torch.complex128, device=self.device)
+        p = self._dev(out, torch.complex128, self.nwf[q] * 4 * self.nxyz) if self.nwf[q] else C.c_void_p()
+        self._chk(self.lib.lise_get_wavefunctions(self._h, q, p), "lise_get_wavefunctions")
+        return out
+
+    def densities(self, q, out=None):
+        if out is None:
+            out = torch.empty((14,) + self.shape, dtype=torch.float64, device=self.device)
+        self._chk(self.lib.lise_densities(self._h, q, self._dev(out, torch.float64, 14 * self.nxyz)), "lise_densities")
+        return out
+
+    def potentials(self, q, out=None):
+        if out is None:
+            out = torch.empty((14,) + self.shape, dtype=torch.float64, device=self.device)
+        self._chk(self.lib.lise_potentials(self._h, q, self._dev(out, torch.float64, 14 * self.nxyz)), "lise_potentials")
+        return out
+
+    def apply_h(self, q, psi, out=None):
+        nst = psi.numel() // (4 * self.nxyz)
+        if out is None:
+            out = torch.empty_like(psi)
+        self._chk(self.lib.lise_apply_h(self._h, q, self._dev(psi, torch.complex128, nst * 4 * self.nxyz),
+                                        self._dev(out, torch.complex128, nst * 4 * self.nxyz), nst), "lise_apply_h")
+        return out
+
+    def step(self, nsteps=1):
+        self._chk(self.lib.lise_step(self._h, nsteps), "lise_step")
+
+    def observables(self):
+        o = Observables()
+        self._chk(self.lib.lise_observables(self._h, C.byref(o)), "lise_observables")
+        return o.as_dict()
+
+    PROFILE_CLASSES = ("happly_yz", "happly_xz", "update_yz", "dens_x", "grid")
+
+    def profile(self, enable=True):
+        self._chk(self.lib.lise_profile(self._h, int(enable)), "lise_profile")
+
+    def profile_read(self):
+        ms = (C.c_double * 5)(); cnt = (C.c_long * 5)()
+        self._chk(self.lib.lise_profile_read(self._h, ms, cnt), "lise_profile_read")
+        return {n: (ms[i], cnt[i]) for i, n in enumerate(self.PROFILE_CLASSES)}
+
+    def launch_count(self):
+        return int(self.lib.lise_launch_count(self._h))
+
+    def device_bytes(self):
+        return int(self.lib.lise_device_bytes(self._h))

@@ -1,0 +1,146 @@
+"""GPU parity: the CUDA path (through the C-ABI binding) against the CPU oracle, element by element,
+on the same seeded inputs.  Tolerances are BASELINE.json's north_star:
+  wavefunctions <= 1e-10 (max |diff| / max |ref|) after 10 steps, densities <= 1e-11, energy <= 1e-10.
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import ref
+from paper_2009_00745_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+TOL_WF, TOL_DENS, TOL_E = 1e-10, 1e-11, 1e-10
+
+
+def rel(a, b):
+    a = np.asarray(a); b = np.asarray(b)
+    return float(np.abs(a - b).max() / max(np.abs(b).max(), 1e-300))
+
+
+def field_rel(got, want):
+    """per-field max-norm relative error for [nfields, ...] arrays; fields that are identically ~0 in the
+    reference are compared on the scale of the largest field."""
+    scale = np.abs(want).max()
+    out = []
+    for f in range(want.shape[0]):
+        s = np.abs(want[f]).max()
+        out.append(np.abs(got[f] - want[f]).max() / (s if s > 1e-9 * scale else scale))
+    return max(out)
+
+
+CASES = {
+    # name: (config index, shape override, dx override, (nwf_n, nwf_p), steps)
+    "config0": (0, None, None, (128, 0), 10),                  # BASELINE configs[0] in full
+    "both_12x8x16": (0, (12, 8, 16), 1.5, (20, 12), 10),       # non-cubic, both species, Coulomb, ragged chunks
+    "r2_6x10x12": (0, (6, 10, 12), 1.5, (7, 5), 6),            # sizes not divisible by 4 (R = 2 blocking)
+    "c1_24c": (1, None, None, (16, 16), 10),                   # configs[1] lattice, reduced states
+    "c2_32c": (2, None, None, (6, 6), 5),
+    "c3_24x24x64": (3, None, None, (4, 4), 4),
+    "c4_40c": (4, None, None, (3, 3), 4),
+}
+
+
+def make_case(name):
+    from paper_2009_00745_b200 import lise
+    idx, shape, dx, nwf, steps = CASES[name]
+    cfg = dict(inputs.CONFIGS[idx])
+    if shape is not None:
+        cfg["shape"] = shape
+    if dx is not None:
+        cfg["dx"] = dx
+    psi = [inputs.make_species(cfg, q, nwf[q], seed=inputs.SEED0 + idx) for q in (0, 1)]
+    oc = ref.RefContext(*cfg["shape"], cfg["dx"], cfg["dt"], nwf[0], nwf[1])
+    gc = lise.Lise(*cfg["shape"], cfg["dx"], cfg["dt"], nwf[0], nwf[1])
+    for q in (0, 1):
+        oc.set_wavefunctions(q, psi[q].numpy())
+        gc.set_wavefunctions(q, psi[q].cuda())
+    return cfg, psi, oc, gc, steps
+
+
+@pytest.fixture(scope="module", params=list(CASES))
+def case(request):
+    c = make_case(request.param)
+    yield (request.param,) + c
+    c[3].close(); c[2].close()
+
+
+def test_initial_densities_potentials_and_hpsi(case):
+    name, cfg, psi, oc, gc, steps = case
+    for q in (0, 1):
+        if oc.nwf[q] == 0:
+            continue
+        d_ref = oc.densities(q); d_gpu = gc.densities(q).cpu().numpy()
+        assert field_rel(d_gpu, d_ref) < TOL_DENS, (name, "densities", q)
+        p_ref = oc.potentials(q); p_gpu = gc.potentials(q).cpu().numpy()
+        assert field_rel(p_gpu, p_ref) < 1e-10, (name, "potentials", q)
+        h_ref = oc.apply_h(q, psi[q].numpy()).reshape(psi[q].shape)
+        h_gpu = gc.apply_h(q, psi[q].cuda()).cpu().numpy()
+        assert rel(h_gpu, h_ref) < 1e-12, (name, "H psi", q)
+    o_ref = oc.observables(); o_gpu = gc.observables()
+    assert abs(o_gpu["energy"] - o_ref["energy"]) < TOL_E * abs(o_ref["energy"])
+    for k in ("e_kin", "e_skyrme", "e_coul", "e_pair", "n_neutron", "n_proton"):
+        assert abs(o_gpu[k] - o_ref[k]) < TOL_E * max(abs(o_ref[k]), abs(o_ref["energy"])), (name, k)
+    assert o_gpu["norm_defect"] < 1e-12 and o_gpu["ortho_defect"] < 1e-12
+
+
+def test_time_steps_match_oracle(case):
+    name, cfg, psi, oc, gc, steps = case
+    oc.step(steps); gc.step(steps)
+    for q in (0, 1):
+        if oc.nwf[q] == 0:
+            continue
+        w_ref = oc.get_wavefunctions(q); w_gpu = gc.get_wavefunctions(q).cpu().numpy()
+        assert rel(w_gpu, w_ref) < TOL_WF, (name, "wavefunctions", q)
+        assert field_rel(gc.densities(q).cpu().numpy(), oc.densities(q)) < TOL_DENS, (name, "densities", q)
+    o_ref = oc.observables(); o_gpu = gc.observables()
+    assert abs(o_gpu["energy"] - o_ref["energy"]) < TOL_E * abs(o_ref["energy"]), (name, o_gpu, o_ref)
+    assert abs(o_gpu["n_neutron"] - o_ref["n_neutron"]) < TOL_E * max(o_ref["n_neutron"], 1.0)
+    assert abs(o_gpu["norm_defect"] - o_ref["norm_defect"]) < 1e-12
+    assert abs(o_gpu["ortho_defect"] - o_ref["ortho_defect"]) < 1e-12
+    assert o_gpu["step"] == steps and abs(o_gpu["time"] - steps * cfg["dt"]) < 1e-12
+
+
+def test_chunk_size_does_not_change_results():
+    """the state-chunking of the launches is an implementation detail: results are bit-identical
+    for states (each state's arithmetic is independent) and equal to round-off for densities."""
+    from paper_2009_00745_b200 import lise
+    cfg = dict(inputs.CONFIGS[0]); cfg["shape"] = (12, 12, 12)
+    psi = inputs.make_species(cfg, 0, 37, seed=5).cuda()
+    res = []
+    for chunk in (0, 5, 37):
+        g = lise.Lise(*cfg["shape"], cfg["dx"], 0.05, 37, 0)
+        g.set_chunk(chunk)
+        g.set_wavefunctions(0, psi)
+        g.step(5)
+        res.append((g.get_wavefunctions(0).cpu().numpy(), g.densities(0).cpu().numpy()))
+        g.close()
+    for w, d in res[1:]:
+        assert rel(w, res[0][0]) < 1e-13
+        assert rel(d, res[0][1]) < 1e-13
+
+
+def test_edge_cases_and_errors():
+    from paper_2009_00745_b200 import lise
+    import ctypes as C
+    lib = lise.load()
+    h = C.c_void_p()
+    assert lib.lise_create(12, 12, 11, 1.0, 0.05, 4, 0, C.byref(h)) == -1          # odd lattice size
+    assert lib.lise_create(12, 12, 12, -1.0, 0.05, 4, 0, C.byref(h)) == -1         # bad spacing
+    assert lib.lise_create(12, 12, 12, 1.0, 0.05, 4, 0, None) == -1
+    g = lise.Lise(12, 12, 12, 1.5, 0.05, 4, 3)
+    with pytest.raises(lise.LiseError):
+        g.step(1)                                                                    # wavefunctions not set
+    with pytest.raises(lise.LiseError):
+        g.densities(0)
+    g.close()
+    # empty proton species and zero steps are fine
+    cfg = dict(inputs.CONFIGS[0])
+    psi = inputs.make_species(cfg, 0, 3, seed=1).cuda()
+    g = lise.Lise(*cfg["shape"], cfg["dx"], 0.05, 3, 0)
+    g.set_wavefunctions(0, psi)
+    g.step(0)
+    assert torch.equal(g.get_wavefunctions(0), psi)
+    assert float(g.densities(1).abs().max()) == 0.0
+    g.close()
