@@ -1,0 +1,379 @@
+#!/usr/bin/env python
+"""Benchmark of the TDSLDA time step (BASELINE.json metric: qp-wavefunction updates/sec, fp64).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config I]
+
+A "step" is one Adams-Bashforth-Milne predictor-modifier-corrector step (two H evaluations, two density
+barriers, Eq. 78) of EVERY quasiparticle state of both species of the workload; the starter
+(3 series-expansion steps) and lise_observables are outside the timed region.  value = states x K / time.
+N > 1 (torchrun, one rank per GPU): weak scaling, every rank owns the full per-GPU state count, one
+NCCL all-reduce of the density accumulators per barrier.  `--impl reference` times the CPU oracle
+(oracle/, as it stands) on a bounded sample of the same workload on the host cores.
+"""
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "qp-wavefunction updates/sec (fp64 TDSLDA steps)"
+UNIT = "qpwf-updates/s"
+
+
+def read_peaks():
+    """measured denominators written by the driver, else the fallback of B200_PROFILING.md."""
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush(); self.f.seek(0)
+        sm, mx, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            parts = [x.strip() for x in line.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1])); pw.append(float(parts[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, parts[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        self.f.close()
+        try:
+            os.unlink(self.f.name)
+        except OSError:
+            pass
+        if sm:
+            sm.sort()
+            out.update(sm_mhz=sm[len(sm) // 2], sm_max_mhz=max(mx), reasons=sorted(reasons), samples=len(sm),
+                       power_w_max=max(pw))
+        return out
+
+
+def workload(idx, nwf_override=None):
+    from paper_2009_00745_b200 import inputs
+    cfg = dict(inputs.CONFIGS[idx])
+    nwf = tuple(nwf_override) if nwf_override else tuple(cfg["nwf"])
+    return cfg, nwf
+
+
+def make_shard(cfg, q, nwf_total, first, count, seed, device):
+    """this rank's states of species q: occupancy from the GLOBAL count, orthonormalised within the shard."""
+    import torch
+    from paper_2009_00745_b200 import inputs
+    if count == 0:
+        return torch.zeros((0, 4) + tuple(cfg["shape"]), dtype=torch.complex128, device=device)
+    psi = torch.empty((count, 4) + tuple(cfg["shape"]), dtype=torch.complex128, device=device)
+    for f in range(0, count, 256):
+        c = min(256, count - f)
+        psi[f:f + c] = inputs.raw_states(cfg, q, nwf_total, seed, device, first=first + f, count=c)
+    return inputs.orthonormalise(psi, cfg["dx"] ** 3)
+
+
+# per-kernel-class algorithmic traffic in units of one state array S = 64 Nxyz bytes per state processed,
+# and fp64 instructions (DFMA-pipe issue slots) per lattice point per state processed (kernel table)
+def class_model(shape, line_op):
+    nx, ny, nz = shape
+    if line_op == "dense":
+        # circulant sums: 8 N pipe slots per point per component for each of the two line passes of an axis
+        happly_yz = 4 * 16 * (ny + nz) + 4 * 60
+        happly_xz = 4 * 16 * nx + 4 * 30
+        dens_yz = 2 * 8 * (ny + nz) + 60
+        dens_x = 2 * 8 * nx + 30
+    else:
+        def fft(n):     # ~ pipe slots per point of one length-n transform (radix-4/2/3/5 mix), DESIGN.md
+            return 2.8 * math.log2(n)
+        happly_yz = 4 * 6 * (fft(ny) + fft(nz)) + 4 * 60
+        happly_xz = 4 * 6 * fft(nx) + 4 * 30
+        dens_yz = 2 * 3 * (fft(ny) + fft(nz)) + 60
+        dens_x = 2 * 3 * fft(nx) + 30
+    return {
+        "happly_yz": dict(S=2.0, slots=happly_yz),                 # read X, write W
+        "happly_xz": dict(S=3.0, slots=happly_xz),                 # read X, W; write W
+        "update_yz": dict(S=8.5, slots=dens_yz + 40),              # evaluation 1: 11 S, evaluation 2: 6 S -> mean 8.5
+        "dens_x": dict(S=0.5, slots=dens_x),                       # read v_up, v_dn of the new state
+        "grid": dict(S=0.0, slots=0.0),
+    }
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2009_00745_b200 import inputs, lise, sharding
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    if args.gpus != world and rank == 0:
+        print(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}; using {world}", file=sys.stderr)
+
+    cfg, nwf = workload(args.config, args.nwf)
+    shape = tuple(cfg["shape"]); nxyz = shape[0] * shape[1] * shape[2]
+    S = 64.0 * nxyz
+    # capacity rule: 7 resident state arrays + scratch must fit; shrink to a multiple of 256 if not
+    free, total = torch.cuda.mem_get_info(dev)
+    per_state = 7 * S
+    cap = int((free - 8 * 2 ** 30) / per_state)
+    req = nwf
+    if nwf[0] + nwf[1] > cap:
+        each = max(256, (cap // 2) // 256 * 256)
+        nwf = (min(nwf[0], each), min(nwf[1], each))
+    tot = (nwf[0] * world, nwf[1] * world)                      # weak scaling: global counts
+    seed = inputs.SEED0 + args.config
+
+    t0 = time.time()
+    g = lise.Lise(*shape, cfg["dx"], cfg["dt"], nwf[0], nwf[1])
+    if world > 1:
+        sharding.attach(g)
+    host = []
+    for q in (0, 1):
+        first = rank * nwf[q]
+        psi = make_shard(cfg, q, tot[q], first, nwf[q], seed, dev)
+        g.set_wavefunctions(q, psi)
+        if args.e2e and nwf[q]:
+            h = torch.empty(psi.shape, dtype=torch.complex128, pin_memory=True)
+            host.append(h)
+        else:
+            host.append(None)
+        del psi
+    torch.cuda.synchronize()
+    t_setup = time.time() - t0
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    nstates = nwf[0] + nwf[1]
+    g.step(3)                                   # series-expansion starter: outside the timed region
+    for _ in range(args.warmup):
+        g.step(1)
+    barrier()
+    l0 = g.launch_count()
+    sampler = ClockSampler(local) if rank == 0 else None
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    wall0 = time.time()
+    ev0.record()
+    g.step(args.steps)
+    ev1.record()
+    barrier()
+    wall = time.time() - wall0
+    ms = ev0.elapsed_time(ev1)
+    launches = g.launch_count() - l0
+    clocks = sampler.stop() if sampler else None
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t[0])
+    value = nstates * world * args.steps / (ms * 1e-3)
+    obs = g.observables()
+
+    # ---- per-kernel-class device times (CUDA events inside the library, on the launching stream) ----
+    g.profile(True)
+    g.step(max(1, min(args.steps, 2)))
+    prof = g.profile_read()
+    g.profile(False)
+    psteps = max(1, min(args.steps, 2))
+
+    # ---- end to end through the C-ABI with HOST buffers ----
+    e2e = None
+    if args.e2e:
+        for q in (0, 1):
+            if host[q] is not None:
+                g.download_wavefunctions(q, host[q])            # host mirror of y_n
+        barrier()
+        w0 = time.time()
+        for _ in range(args.steps):
+            for q in (0, 1):
+                if host[q] is not None:
+                    g.upload_wavefunctions(q, host[q], keep_history=True)   # H2D of the step's input
+            g.step(1)
+            for q in (0, 1):
+                if host[q] is not None:
+                    g.download_wavefunctions(q, host[q])        # D2H of the step's result (y_{n+1}); synchronises
+        barrier()
+        w = time.time() - w0
+        if world > 1:
+            t = torch.tensor([w], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            w = float(t[0])
+        nbytes = sum(h.numel() * 16 for h in host if h is not None)
+        e2e = {"value": nstates * world * args.steps / w, "unit": UNIT,
+               "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes}
+
+    if rank != 0:
+        g.close()
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- rooflines ----
+    hbm_gbs, hbm_src = read_peaks()
+    fp64_tf = lise.measure_fp64_peak(1.5)
+    line_op = os.environ.get("LISE_LINE_OP", lise.line_operator(g) if hasattr(lise, "line_operator") else "dense")
+    model = class_model(shape, line_op)
+    tot_ms = sum(v[0] for v in prof.values())
+    top = max((k for k in prof if k != "grid"), key=lambda k: prof[k][0])
+    top_ms, top_n = prof[top]
+    states_per_launch = nstates * psteps * 2.0 / max(top_n, 1)       # every state passes each class twice per step
+    bytes_per_launch = model[top]["S"] * S * states_per_launch
+    slots_per_launch = model[top]["slots"] * nxyz * states_per_launch
+    avg_s = top_ms * 1e-3 / max(top_n, 1)
+    t_hbm = bytes_per_launch / (hbm_gbs * 1e9)
+    t_alu = slots_per_launch * 2.0 / (fp64_tf * 1e12)
+    if t_alu > t_hbm:
+        roof = {"bound": "alu", "achieved": slots_per_launch * 2.0 / avg_s * 1e-12, "peak": fp64_tf, "unit": "TFLOP/s",
+                "peak_source": "measured here: DFMA microbenchmark (lise_measure_fp64_peak), 2 flop per fp64 pipe slot"}
+    else:
+        roof = {"bound": "hbm", "achieved": bytes_per_launch / avg_s * 1e-9, "peak": hbm_gbs, "unit": "GB/s",
+                "peak_source": hbm_src}
+    roof["frac"] = roof["achieved"] / roof["peak"]
+    roof["kernel"] = top
+    roof["avg_launch_ms"] = avg_s * 1e3
+    roof["share_of_step"] = top_ms / tot_ms if tot_ms > 0 else None
+    roof["traffic"] = None
+    roof["classes_ms_per_step"] = {k: v[0] / psteps for k, v in prof.items()}
+    step_bytes = 15.0 * S                                              # B_min = 960 Nxyz per qpwf-update
+    per_gpu = value / world
+    step_roof = {"hbm_bytes_per_update": step_bytes, "hbm_frac_of_measured": per_gpu * step_bytes / (hbm_gbs * 1e9),
+                 "hbm_frac_of_8TBs": per_gpu * step_bytes / 8e12, "hbm_peak_gbs": hbm_gbs, "hbm_peak_source": hbm_src,
+                 "fp64_peak_tflops_measured": fp64_tf}
+
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+           "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+           "dtype": "f64", "data": "synthetic",
+           "config": {"workload": cfg["name"], "lattice": list(shape), "dx_fm": cfg["dx"], "dt_fm_c": cfg["dt"],
+                      "states_per_gpu": list(nwf), "states_requested": list(req), "coulomb": bool(cfg["coulomb"] and nwf[1] > 0),
+                      "parallelism": f"state-sharded x{world}" if world > 1 else "single GPU",
+                      "l2": "inputs larger than L2 (7 state arrays = %.1f GB resident)" % (7 * S * nstates / 1e9),
+                      "line_operator": line_op, "setup_s": round(t_setup, 1)},
+           "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roof, "step_roofline": step_roof,
+           "wall_s_timed_region": wall,
+           "observables": {k: obs[k] for k in ("energy", "n_neutron", "n_proton", "norm_defect", "ortho_defect", "step")}}
+    if args.cpu_baseline and world == 1:
+        out["cpu_baseline"] = cpu_baseline(cfg, args.cpu_states)
+    g.close()
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def oracle_sample(cfg, ns, nsteps, warm=0):
+    """time `nsteps` steady ABM steps of the oracle on ns + ns states of the workload's lattice."""
+    import numpy as np
+    from oracle import ref
+    from paper_2009_00745_b200 import inputs
+    shape = tuple(cfg["shape"])
+    both = cfg["nwf"][1] > 0
+    nwf = (ns, ns if both else 0)
+    oc = ref.RefContext(*shape, cfg["dx"], cfg["dt"], *nwf)
+    for q in (0, 1):
+        if nwf[q] == 0:
+            continue
+        psi = inputs.make_species(cfg, q, nwf[q], seed=inputs.SEED0).numpy()
+        oc.set_wavefunctions(q, psi)
+        z = np.zeros_like(psi)
+        oc.set_history(q, psi, z, z, z, z)        # marks the multistep method as started: next steps are ABM steps
+    cores = ref.set_num_threads(0)
+    if warm:
+        oc.step(warm)
+    t0 = time.time()
+    oc.step(nsteps)
+    dt = time.time() - t0
+    oc.close()
+    return (nwf[0] + nwf[1]) * nsteps / dt, dt, cores, nwf
+
+
+def cpu_baseline(cfg, ns):
+    v, dt, cores, nwf = oracle_sample(cfg, ns, 1)
+    return {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{nwf[0]}+{nwf[1]} states x 1 ABM step on the {cfg['name']} lattice ({dt:.1f} s), history pre-filled"}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cfg, nwf = workload(args.config, args.nwf)
+    ns = args.cpu_states
+    t0 = time.time()
+    v, dt, cores, snwf = oracle_sample(cfg, ns, args.steps, warm=args.warmup)
+    out = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": int(os.environ.get("WORLD_SIZE", "1")),
+           "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3 / args.steps, "higher_is_better": True,
+           "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": cfg["name"], "lattice": list(cfg["shape"]), "dx_fm": cfg["dx"], "dt_fm_c": cfg["dt"],
+                      "states_per_gpu": list(nwf), "sample_states": list(snwf)},
+           "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+                            "sample": f"{snwf[0]}+{snwf[1]} states per step, {args.steps} ABM steps after {args.warmup} warm-up"},
+           "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0, "wall_s": time.time() - t0}
+    print(json.dumps(out))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs (default 1: the 24^3 workload)")
+    ap.add_argument("--nwf", type=int, nargs=2, default=None, help="override states per species per GPU (testing)")
+    ap.add_argument("--no-e2e", dest="e2e", action="store_false")
+    ap.add_argument("--no-cpu-baseline", dest="cpu_baseline", action="store_false")
+    ap.add_argument("--cpu-states", type=int, default=0, help="oracle sample: states per species (0 = sized from the host core count)")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        print("bench.py: warm-up raised to 3 (timing rules)", file=sys.stderr)
+        args.warmup = 3
+    if args.cpu_states <= 0:
+        cores = os.cpu_count() or 4
+        # the oracle costs about 0.5 core-seconds per qpwf-update on the 24^3 lattice: ~12 s for the
+        # cpu_baseline sample, ~2 s per step for the reference arm (W + K steps)
+        args.cpu_states = min(512, 12 * cores) if args.impl == "ours" else min(256, 2 * cores)
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

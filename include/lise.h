@@ -85,6 +85,15 @@ int lise_set_chunk(lise_ctx *ctx, int nstates);
 int lise_set_wavefunctions(lise_ctx *ctx, int species, const void *psi_dev);
 int lise_get_wavefunctions(lise_ctx *ctx, int species, void *psi_dev);
 
+/* HOST-buffer variants (psi_host is a HOST pointer, pinned or pageable, same layout): the copy is
+ * enqueued on the context's stream with cudaMemcpyAsync.  lise_upload_wavefunctions with
+ * keep_history = 0 is lise_set_wavefunctions from host memory; with keep_history = 1 it overwrites
+ * y_n only (restoring a host mirror of the current wavefunctions, e.g. after a checkpoint,
+ * PAPER.md:L764-L768), re-accumulates their densities and keeps the multistep history, step counter
+ * and time.  lise_download_wavefunctions copies y_n out and returns after the stream has drained. */
+int lise_upload_wavefunctions(lise_ctx *ctx, int species, const void *psi_host, int keep_history);
+int lise_download_wavefunctions(lise_ctx *ctx, int species, void *psi_host);
+
 /* Local densities of the current wavefunctions of one species in the layout of the paper's
  * d_densities (Table 2): 14*Nxyz doubles = n, tau, s(3), div J, j(3), curl j(3),
  * kappa (re, im).  Eq. 3 with tau via Eq. 51. */
@@ -105,6 +114,15 @@ int lise_apply_h(lise_ctx *ctx, int species, const void *in_dev, void *out_dev, 
  * the phase removal of Eqs. 80-81. */
 int lise_step(lise_ctx *ctx, int nsteps);
 
+/* State-sharded multi-GPU runs (one process per GPU: each rank owns nwf/G states,
+ * grid fields replicated): the hook is called on the host at each of the two density barriers of a
+ * step, after this rank's partial accumulators have been summed into `acc_dev` (DEVICE pointer,
+ * `count` doubles = 2 species x 13 accumulators x Nxyz, work already enqueued on the context's
+ * stream).  It must enqueue an in-place sum over ranks of acc_dev on the same stream (e.g. an NCCL
+ * all-reduce) and return 0; a non-zero return aborts the step with LISE_ECUDA.  NULL removes the hook. */
+typedef int (*lise_reduce_fn)(void *user, double *acc_dev, long count);
+int lise_set_reduce_hook(lise_ctx *ctx, lise_reduce_fn fn, void *user);
+
 /* Energy, particle numbers, norm / orthonormality defects of the current wavefunctions. Synchronises. */
 int lise_observables(lise_ctx *ctx, lise_observables_t *host_out);
 
@@ -117,6 +135,12 @@ int lise_observables(lise_ctx *ctx, lise_observables_t *host_out);
  * ms and counts are HOST arrays of 5 entries. */
 int lise_profile(lise_ctx *ctx, int enable);
 int lise_profile_read(lise_ctx *ctx, double *ms, long *counts);
+
+/* Measures the fp64 FMA throughput of the current device (the denominator of the "alu" roofline): runs a
+ * register-only DFMA kernel back to back on `stream` (cudaStream_t, may be NULL) for about `seconds`
+ * and writes the best TFLOP/s (2 flop per FMA) seen in the second half of that time to *tflops_host
+ * (HOST pointer).  sm_mhz_host is reserved (set to 0).  Synchronises. */
+int lise_measure_fp64_peak(void *stream, double seconds, double *tflops_host, double *sm_mhz_host);
 
 /* Number of kernel launches issued by this context so far (for bench.py's gpu_launches). */
 long lise_launch_count(const lise_ctx *ctx);

@@ -30,8 +30,20 @@ class Observables(C.Structure):
 
 EXPORTS = ["lise_default_params", "lise_create", "lise_destroy", "lise_set_params", "lise_set_stream",
            "lise_set_dt", "lise_set_chunk", "lise_set_wavefunctions", "lise_get_wavefunctions",
+           "lise_upload_wavefunctions", "lise_download_wavefunctions", "lise_set_reduce_hook",
            "lise_densities", "lise_potentials", "lise_apply_h", "lise_step", "lise_observables",
-           "lise_profile", "lise_profile_read", "lise_launch_count", "lise_device_bytes", "lise_strerror", "lise_last_error"]
+           "lise_profile", "lise_profile_read", "lise_measure_fp64_peak", "lise_launch_count", "lise_device_bytes", "lise_strerror", "lise_last_error"]
+
+
+REDUCE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_long)
+
+
+class _DevView:
+    """__cuda_array_interface__ wrapper of a raw device pointer (float64), for torch.as_tensor."""
+
+    def __init__(self, ptr, count):
+        self.__cuda_array_interface__ = {"shape": (count,), "typestr": "<f8", "data": (ptr, False), "version": 3,
+                                         "strides": None}
 
 
 def lib_path():
@@ -59,6 +71,9 @@ def load():
     lib.lise_set_chunk.argtypes = [vp, ip]
     lib.lise_set_wavefunctions.argtypes = [vp, ip, vp]
     lib.lise_get_wavefunctions.argtypes = [vp, ip, vp]
+    lib.lise_upload_wavefunctions.argtypes = [vp, ip, vp, ip]
+    lib.lise_download_wavefunctions.argtypes = [vp, ip, vp]
+    lib.lise_set_reduce_hook.argtypes = [vp, REDUCE_FN, vp]
     lib.lise_densities.argtypes = [vp, ip, vp]
     lib.lise_potentials.argtypes = [vp, ip, vp]
     lib.lise_apply_h.argtypes = [vp, ip, vp, vp, ip]
@@ -66,6 +81,7 @@ def load():
     lib.lise_observables.argtypes = [vp, C.POINTER(Observables)]
     lib.lise_profile.argtypes = [vp, ip]
     lib.lise_profile_read.argtypes = [vp, C.POINTER(dp), C.POINTER(C.c_long)]
+    lib.lise_measure_fp64_peak.argtypes = [vp, dp, C.POINTER(dp), C.POINTER(dp)]
     lib.lise_launch_count.argtypes = [vp]; lib.lise_launch_count.restype = C.c_long
     lib.lise_device_bytes.argtypes = [vp]; lib.lise_device_bytes.restype = C.c_longlong
     lib.lise_strerror.argtypes = [ip]; lib.lise_strerror.restype = C.c_char_p
@@ -78,6 +94,18 @@ def default_params():
     p = Params()
     load().lise_default_params(C.byref(p))
     return p
+
+
+def measure_fp64_peak(seconds=1.0, stream=None):
+    """sustained fp64 FMA throughput of the current device in TFLOP/s (DFMA microbenchmark)."""
+    if not torch.cuda.is_available():
+        raise RuntimeError("no CUDA device")
+    st = torch.cuda.current_stream() if stream is None else stream
+    tf = C.c_double(); mhz = C.c_double()
+    rc = load().lise_measure_fp64_peak(C.c_void_p(st.cuda_stream), seconds, C.byref(tf), C.byref(mhz))
+    if rc != 0:
+        raise RuntimeError(f"lise_measure_fp64_peak failed ({rc})")
+    return tf.value
 
 
 class LiseError(RuntimeError):
@@ -152,6 +180,39 @@ class Lise:
         p = self._dev(out, torch.complex128, self.nwf[q] * 4 * self.nxyz) if self.nwf[q] else C.c_void_p()
         self._chk(self.lib.lise_get_wavefunctions(self._h, q, p), "lise_get_wavefunctions")
         return out
+
+    def _host(self, t, numel):
+        if not (t.device.type == "cpu" and t.dtype == torch.complex128 and t.is_contiguous() and t.numel() == numel):
+            raise LiseError(f"expected a contiguous CPU complex128 tensor with {numel} elements")
+        return C.c_void_p(t.data_ptr())
+
+    def upload_wavefunctions(self, q, psi_host, keep_history=False):
+        """host tensor (pinned for speed) -> y_n of species q, through the library's own H2D copy."""
+        p = self._host(psi_host, self.nwf[q] * 4 * self.nxyz) if self.nwf[q] else C.c_void_p()
+        self._chk(self.lib.lise_upload_wavefunctions(self._h, q, p, int(keep_history)), "lise_upload_wavefunctions")
+
+    def download_wavefunctions(self, q, out_host):
+        p = self._host(out_host, self.nwf[q] * 4 * self.nxyz) if self.nwf[q] else C.c_void_p()
+        self._chk(self.lib.lise_download_wavefunctions(self._h, q, p), "lise_download_wavefunctions")
+        return out_host
+
+    def set_reduce_hook(self, reduce_tensor):
+        """reduce_tensor(t): in-place sum over ranks of the float64 CUDA tensor t, enqueued on the
+        context's stream (e.g. lambda t: torch.distributed.all_reduce(t)).  None removes the hook."""
+        if reduce_tensor is None:
+            self._hook = None
+            self._chk(self.lib.lise_set_reduce_hook(self._h, REDUCE_FN(0), None), "lise_set_reduce_hook")
+            return
+
+        def _cb(user, ptr, count):
+            try:
+                reduce_tensor(torch.as_tensor(_DevView(ptr, count), device=self.device))
+                return 0
+            except Exception as exc:  # never let an exception cross the C ABI
+                self._hook_error = exc
+                return 1
+        self._hook = REDUCE_FN(_cb)     # keep alive
+        self._chk(self.lib.lise_set_reduce_hook(self._h, self._hook, None), "lise_set_reduce_hook")
 
     def densities(self, q, out=None):
         if out is None:
