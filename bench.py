@@ -96,11 +96,7 @@ def make_shard(cfg, q, nwf_total, first, count, seed, device):
     from paper_2009_00745_b200 import inputs
     if count == 0:
         return torch.zeros((0, 4) + tuple(cfg["shape"]), dtype=torch.complex128, device=device)
-    psi = torch.empty((count, 4) + tuple(cfg["shape"]), dtype=torch.complex128, device=device)
-    for f in range(0, count, 256):
-        c = min(256, count - f)
-        psi[f:f + c] = inputs.raw_states(cfg, q, nwf_total, seed, device, first=first + f, count=c)
-    return inputs.orthonormalise(psi, cfg["dx"] ** 3)
+    return inputs.make_block(cfg, q, nwf_total, first, count, seed, device)
 
 
 # per-kernel-class algorithmic traffic in units of one state array S = 64 Nxyz bytes per state processed,
@@ -249,7 +245,7 @@ def run_ours(args):
     # ---- rooflines ----
     hbm_gbs, hbm_src = read_peaks()
     fp64_tf = lise.measure_fp64_peak(1.5)
-    line_op = os.environ.get("LISE_LINE_OP", lise.line_operator(g) if hasattr(lise, "line_operator") else "dense")
+    line_op = g.line_operator()
     model = class_model(shape, line_op)
     tot_ms = sum(v[0] for v in prof.values())
     top = max((k for k in prof if k != "grid"), key=lambda k: prof[k][0])

@@ -142,6 +142,11 @@ int lise_profile_read(lise_ctx *ctx, double *ms, long *counts);
  * (HOST pointer).  sm_mhz_host is reserved (set to 0).  Synchronises. */
 int lise_measure_fp64_peak(void *stream, double seconds, double *tflops_host, double *sm_mhz_host);
 
+/* Which line operator the per-state kernels of this context use: "dmma" (fp64 tensor-core tiles, for the
+ * lattice shapes the library was instantiated for; LISE_LINE_OP=dense in the environment disables it)
+ * or "dense" (generic DFMA circulant sums, any even lattice).  Both apply the same operator (Eq. 48). */
+const char *lise_line_operator(const lise_ctx *ctx);
+
 /* Number of kernel launches issued by this context so far (for bench.py's gpu_launches). */
 long lise_launch_count(const lise_ctx *ctx);
 /* Bytes of device memory held by the context. */

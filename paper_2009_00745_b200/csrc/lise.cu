@@ -15,6 +15,15 @@
 
 enum { RA = 0, RB, RC, RD, RE, RF, RG };
 
+typedef void (*HKern)(HArgs);
+typedef void (*UKern)(UArgs);
+typedef void (*DKern)(DArgs);
+struct KernSet {
+    HKern h_yz, h_xz;
+    UKern u[4];
+    DKern d_x;
+    const char* name;
+};
 struct lise_ctx {
     Lattice L;
     int n[3];
@@ -38,7 +47,8 @@ struct lise_ctx {
     cplx *tw, *cA1, *cA2, *cA3;
     double* ebuf; int eblocks;
     cplx* ovl;
-    int R, thr[2];
+    int R, thr[2], mma;
+    KernSet ks;
     size_t smem_h[2], smem_u, smem_d;
     int have[2], pot_valid;
     long step; double time;
@@ -148,18 +158,41 @@ extern "C" int lise_default_params(lise_params* p)
     return LISE_OK;
 }
 
-// ---- kernel launch helpers (dispatch on the register blocking R) ----
+// ---- kernel sets: the plane kernels instantiated for one line-operator policy per plane kind ----
+template <class LOYZ, class LOXZ>
+static KernSet make_set(const char* name)
+{
+    KernSet k;
+    k.h_yz = k_happly<0, LOYZ>; k.h_xz = k_happly<1, LOXZ>;
+    k.u[0] = k_update_yz<0, LOYZ>; k.u[1] = k_update_yz<1, LOYZ>; k.u[2] = k_update_yz<2, LOYZ>; k.u[3] = k_update_yz<3, LOYZ>;
+    k.d_x = k_dens_x<LOXZ>;
+    k.name = name;
+    return k;
+}
+// DMMA line operators exist for these (nx; ny, nz) combinations (every lattice of BASELINE.json's configs
+// except the 12^3 one of config 0 ... which is listed too); anything else runs the generic DFMA kernels.
+#define LISE_MMA_SHAPES(X) \
+    X(8, 8, 8) X(12, 12, 12) X(16, 16, 16) X(20, 20, 20) X(24, 24, 24) X(32, 32, 32) X(40, 40, 40) X(48, 48, 48) X(64, 64, 64) \
+    X(24, 24, 48) X(24, 24, 64) X(12, 8, 16) X(16, 12, 8) X(32, 32, 64)
+static bool pick_kernels(int nx, int ny, int nz, int R, bool want_mma, KernSet* out)
+{
+    if (want_mma) {
+#define X(a, b, c_) if (nx == a && ny == b && nz == c_) { *out = make_set<MmaLines<b, c_>, MmaLines<a, 0>>("dmma"); return true; }
+        LISE_MMA_SHAPES(X)
+#undef X
+    }
+    if (R == 8) *out = make_set<DenseLines<8>, DenseLines<8>>("dense");
+    else if (R == 4) *out = make_set<DenseLines<4>, DenseLines<4>>("dense");
+    else *out = make_set<DenseLines<2>, DenseLines<2>>("dense");
+    return false;
+}
+
 template <int KIND>
 static int launch_happly(lise_ctx* c, const HArgs& a)
 {
     dim3 grid(KIND == 0 ? c->L.nx : c->L.ny, c->G);
-    const int t = c->thr[KIND]; const size_t sm = c->smem_h[KIND];
     prof_begin(c, KIND == 0 ? PC_HAPPLY_YZ : PC_HAPPLY_XZ);
-    switch (c->R) {
-    case 8: k_happly<KIND, 8><<<grid, t, sm, c->stream>>>(a); break;
-    case 4: k_happly<KIND, 4><<<grid, t, sm, c->stream>>>(a); break;
-    default: k_happly<KIND, 2><<<grid, t, sm, c->stream>>>(a); break;
-    }
+    (KIND == 0 ? c->ks.h_yz : c->ks.h_xz)<<<grid, c->thr[KIND], c->smem_h[KIND], c->stream>>>(a);
     prof_end(c);
     CKL();
     return LISE_OK;
@@ -168,13 +201,8 @@ template <int MODE>
 static int launch_update(lise_ctx* c, const UArgs& a)
 {
     dim3 grid(c->L.nx, c->G);
-    const int t = c->thr[0]; const size_t sm = c->smem_u;
     prof_begin(c, PC_UPDATE);
-    switch (c->R) {
-    case 8: k_update_yz<MODE, 8><<<grid, t, sm, c->stream>>>(a); break;
-    case 4: k_update_yz<MODE, 4><<<grid, t, sm, c->stream>>>(a); break;
-    default: k_update_yz<MODE, 2><<<grid, t, sm, c->stream>>>(a); break;
-    }
+    c->ks.u[MODE]<<<grid, c->thr[0], c->smem_u, c->stream>>>(a);
     prof_end(c);
     CKL();
     return LISE_OK;
@@ -182,32 +210,18 @@ static int launch_update(lise_ctx* c, const UArgs& a)
 static int launch_dens_x(lise_ctx* c, const DArgs& a)
 {
     dim3 grid(c->L.ny, c->G);
-    const int t = c->thr[1]; const size_t sm = c->smem_d;
     prof_begin(c, PC_DENS_X);
-    switch (c->R) {
-    case 8: k_dens_x<8><<<grid, t, sm, c->stream>>>(a); break;
-    case 4: k_dens_x<4><<<grid, t, sm, c->stream>>>(a); break;
-    default: k_dens_x<2><<<grid, t, sm, c->stream>>>(a); break;
-    }
+    c->ks.d_x<<<grid, c->thr[1], c->smem_d, c->stream>>>(a);
     prof_end(c);
     CKL();
     return LISE_OK;
 }
-template <typename K>
-static cudaError_t set_smem(K kern, size_t bytes)
-{
-    return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
-}
-template <int R>
 static int set_attrs(lise_ctx* c)
 {
-    CK(set_smem(k_happly<0, R>, c->smem_h[0]));
-    CK(set_smem(k_happly<1, R>, c->smem_h[1]));
-    CK(set_smem(k_update_yz<0, R>, c->smem_u));
-    CK(set_smem(k_update_yz<1, R>, c->smem_u));
-    CK(set_smem(k_update_yz<2, R>, c->smem_u));
-    CK(set_smem(k_update_yz<3, R>, c->smem_u));
-    CK(set_smem(k_dens_x<R>, c->smem_d));
+    CK(cudaFuncSetAttribute(c->ks.h_yz, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_h[0]));
+    CK(cudaFuncSetAttribute(c->ks.h_xz, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_h[1]));
+    for (int m = 0; m < 4; ++m) CK(cudaFuncSetAttribute(c->ks.u[m], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_u));
+    CK(cudaFuncSetAttribute(c->ks.d_x, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_d));
     return LISE_OK;
 }
 
@@ -475,11 +489,15 @@ static int ctx_init(lise_ctx* c)
         int r = atoi(e);
         if ((r == 2 || r == 4 || r == 8) && L.nx % r == 0 && L.ny % r == 0 && L.nz % r == 0) c->R = r;
     }
+    bool want_mma = true;
+    if (const char* e = getenv("LISE_LINE_OP")) want_mma = (strcmp(e, "dense") != 0);
+    c->mma = pick_kernels(L.nx, L.ny, L.nz, c->R, want_mma, &c->ks) ? 1 : 0;
     const int ld = L.nz + 1;
     const int n1[2] = {L.ny, L.nx};
     for (int k = 0; k < 2; ++k) {
         const int npts = n1[k] * L.nz;
-        int t = ((2 * npts / c->R + 31) / 32) * 32;
+        int t = c->mma ? 256 : ((2 * npts / c->R + 31) / 32) * 32;
+        if (c->mma && npts <= 256) t = 128;
         if (t > 512) t = 512;
         if (t < 64) t = 64;
         c->thr[k] = t;
@@ -493,7 +511,7 @@ static int ctx_init(lise_ctx* c)
                  c->smem_h[0] > c->smem_h[1] ? c->smem_h[0] : c->smem_h[1], lim);
         return LISE_EUNSUPPORTED;
     }
-    if (c->R == 8) TRY(set_attrs<8>(c)); else if (c->R == 4) TRY(set_attrs<4>(c)); else TRY(set_attrs<2>(c));
+    TRY(set_attrs(c));
     int minp = L.nx < L.ny ? L.nx : L.ny;
     c->G = (2 * 148 + minp - 1) / minp;
     if (c->G > LISE_MAXG) c->G = LISE_MAXG;
@@ -814,6 +832,8 @@ extern "C" int lise_measure_fp64_peak(void* stream, double seconds, double* tflo
     if (sm_mhz_host) *sm_mhz_host = 0.0;
     return rc;
 }
+
+extern "C" const char* lise_line_operator(const lise_ctx* c) { return c ? c->ks.name : "none"; }
 
 extern "C" long lise_launch_count(const lise_ctx* c) { return c ? c->launches : 0; }
 extern "C" long long lise_device_bytes(const lise_ctx* c) { return c ? c->bytes : 0; }

@@ -20,14 +20,22 @@ CONFIGS = [
     dict(name="config0_12c_n128", shape=(12, 12, 12), dx=1.5, dt=0.05, steps=10, nwf=(128, 0),
          kc=0.8, w=4.0, centres=[(0.0, 0.0, 0.0)], occ=(0.5, 0.5), coulomb=False),
     dict(name="config1_24c", shape=(24, 24, 24), dx=1.25, dt=0.05, steps=100, nwf=(4096, 4096),
-         kc=1.5, w=5.0, centres=[(0.0, 0.0, 0.0)], occ=None, coulomb=True),
+         kc=2.0, w=5.0, centres=[(0.0, 0.0, 0.0)], occ=None, coulomb=True, ortho="split"),
     dict(name="config2_32c", shape=(32, 32, 32), dx=1.25, dt=0.05, steps=100, nwf=(8192, 8192),
-         kc=1.5, w=6.0, centres=[(0.0, 0.0, 0.0)], occ=None, coulomb=True),
+         kc=1.8, w=6.0, centres=[(0.0, 0.0, 0.0)], occ=None, coulomb=True, ortho="split"),
     dict(name="config3_24x24x64", shape=(24, 24, 64), dx=1.25, dt=0.05, steps=200, nwf=(8192, 8192),
-         kc=1.2, w=4.0, centres=[(0.0, 0.0, -12.0), (0.0, 0.0, 12.0)], occ=None, coulomb=True),
+         kc=1.2, w=4.0, centres=[(0.0, 0.0, -12.0), (0.0, 0.0, 12.0)], occ=None, coulomb=True, ortho="split"),
     dict(name="config4_40c", shape=(40, 40, 40), dx=1.0, dt=0.03, steps=100, nwf=(6144, 6144),
-         kc=1.8, w=7.0, centres=[(0.0, 0.0, 0.0)], occ=None, coulomb=True),
+         kc=1.8, w=7.0, centres=[(0.0, 0.0, 0.0)], occ=None, coulomb=True, ortho="split"),
 ]
+# "joint": the whole 4-component states are orthonormalised (BASELINE.json's literal recipe; config 0).
+# "split": the u-pairs and the v-pairs are orthonormalised separately in their 2-component inner
+#   products and recombined with the amplitudes sqrt(1-occ), sqrt(occ).  The set is then orthonormal in
+#   the 4-component inner product as well (modified Gram-Schmidt leaves it unchanged) AND keeps the
+#   particle number nwf*occ.  The joint recipe on thousands of u-dominated states pushes the weight of
+#   the later states into v (measured: 1532 neutrons instead of 63 on config 1, 25x nuclear density,
+#   far outside the ABM stability bound); DESIGN.md "input recipe".  Needs 2 * modes(kc) >= nwf:
+#   kc raised to 2.0 (config 1) and 1.8 (config 2).
 N_PEAK = (0.09, 0.07)  # fm^-3, neutron / proton peak densities (sum = saturation 0.16)
 
 
@@ -94,7 +102,7 @@ def envelope(shape, dx, w, centre, device):
     return env
 
 
-def raw_states(cfg, q, nwf_q, seed, device="cpu", first=0, count=None):
+def raw_states(cfg, q, nwf_q, seed, device="cpu", first=0, count=None, scale=True):
     """un-orthonormalised states [count, 4, nx, ny, nz] complex128 (steps 1-3 of the recipe)."""
     shape, dx = cfg["shape"], cfg["dx"]
     count = nwf_q - first if count is None else count
@@ -114,22 +122,29 @@ def raw_states(cfg, q, nwf_q, seed, device="cpu", first=0, count=None):
         coef = torch.complex(re * mask, im * mask)
         p = torch.fft.ifftn(coef, dim=(-3, -2, -1), norm="forward")   # sum_k a(k) e^{ik.r}
         out += p * envelope(shape, dx, cfg["w"], centre, device)
-    for c in range(4):
-        out[:, c] *= amp[c]
+    if scale:
+        for c in range(4):
+            out[:, c] *= amp[c]
     return out
 
 
 def orthonormalise(psi, dV):
     """Q factor (positive diagonal) of the states in <a|b> = dV sum conj(a) b, i.e. the result of
-    modified Gram-Schmidt in state order, computed by Cholesky-QR applied twice."""
+    modified Gram-Schmidt in state order, computed by Cholesky-QR applied three times (Householder QR
+    if the Gram matrix is numerically singular)."""
     n = psi.shape[0]
     a = psi.reshape(n, -1)
-    for _ in range(2):
-        g = (a.conj() @ a.T) * dV          # g[k, l] = <k|l>
-        g = 0.5 * (g + g.conj().T)
-        L = torch.linalg.cholesky(g)       # g = L L^H
-        # rows q_k = sum_l (conj(L)^-1)[k, l] a_l  (lower triangular: MGS order)
-        a = torch.linalg.solve_triangular(L.conj(), a, upper=False)
+    try:
+        for _ in range(3):
+            g = (a.conj() @ a.T) * dV          # g[k, l] = <k|l>
+            g = 0.5 * (g + g.conj().T)
+            L = torch.linalg.cholesky(g)       # g = L L^H
+            # rows q_k = sum_l (conj(L)^-1)[k, l] a_l  (lower triangular: MGS order)
+            a = torch.linalg.solve_triangular(L.conj(), a, upper=False)
+    except Exception:
+        qm, rm = torch.linalg.qr(psi.reshape(n, -1).T)            # columns = states
+        d = torch.diagonal(rm)
+        a = (qm * (d / d.abs()).conj().unsqueeze(0)).T.contiguous() / dV ** 0.5
     return a.reshape(psi.shape)
 
 
@@ -140,11 +155,25 @@ def make_species(cfg, q, nwf_q=None, seed=None, device="cpu", chunk=256):
     shape = tuple(cfg["shape"])
     if nwf_q == 0:
         return torch.zeros((0, 4) + shape, dtype=torch.complex128, device=device)
-    psi = torch.empty((nwf_q, 4) + shape, dtype=torch.complex128, device=device)
-    for f in range(0, nwf_q, chunk):
-        c = min(chunk, nwf_q - f)
-        psi[f:f + c] = raw_states(cfg, q, nwf_q, seed, device, first=f, count=c)
-    return orthonormalise(psi, cfg["dx"] ** 3)
+    return make_block(cfg, q, nwf_q, 0, nwf_q, seed, device, chunk)
+
+
+def make_block(cfg, q, nwf_total, first, count, seed, device="cpu", chunk=256):
+    """states [first, first+count) of a species with nwf_total states in all (the occupancy follows
+    the total), orthonormalised within the block."""
+    shape = tuple(cfg["shape"])
+    dV = cfg["dx"] ** 3
+    split = cfg.get("ortho", "joint") == "split"
+    psi = torch.empty((count, 4) + shape, dtype=torch.complex128, device=device)
+    for f in range(0, count, chunk):
+        c = min(chunk, count - f)
+        psi[f:f + c] = raw_states(cfg, q, nwf_total, seed, device, first=first + f, count=c, scale=not split)
+    if not split:
+        return orthonormalise(psi, dV)
+    occ = occupancy(cfg, q, nwf_total)
+    for half, amp in ((slice(0, 2), math.sqrt(1.0 - occ)), (slice(2, 4), math.sqrt(occ))):
+        psi[:, half] = orthonormalise(psi[:, half].contiguous(), dV) * amp
+    return psi
 
 
 def make_config(idx, nwf=None, device="cpu"):

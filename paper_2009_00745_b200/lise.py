@@ -32,7 +32,7 @@ EXPORTS = ["lise_default_params", "lise_create", "lise_destroy", "lise_set_param
            "lise_set_dt", "lise_set_chunk", "lise_set_wavefunctions", "lise_get_wavefunctions",
            "lise_upload_wavefunctions", "lise_download_wavefunctions", "lise_set_reduce_hook",
            "lise_densities", "lise_potentials", "lise_apply_h", "lise_step", "lise_observables",
-           "lise_profile", "lise_profile_read", "lise_measure_fp64_peak", "lise_launch_count", "lise_device_bytes", "lise_strerror", "lise_last_error"]
+           "lise_profile", "lise_profile_read", "lise_measure_fp64_peak", "lise_line_operator", "lise_launch_count", "lise_device_bytes", "lise_strerror", "lise_last_error"]
 
 
 REDUCE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_long)
@@ -82,6 +82,7 @@ def load():
     lib.lise_profile.argtypes = [vp, ip]
     lib.lise_profile_read.argtypes = [vp, C.POINTER(dp), C.POINTER(C.c_long)]
     lib.lise_measure_fp64_peak.argtypes = [vp, dp, C.POINTER(dp), C.POINTER(dp)]
+    lib.lise_line_operator.argtypes = [vp]; lib.lise_line_operator.restype = C.c_char_p
     lib.lise_launch_count.argtypes = [vp]; lib.lise_launch_count.restype = C.c_long
     lib.lise_device_bytes.argtypes = [vp]; lib.lise_device_bytes.restype = C.c_longlong
     lib.lise_strerror.argtypes = [ip]; lib.lise_strerror.restype = C.c_char_p
@@ -251,6 +252,9 @@ class Lise:
         ms = (C.c_double * 5)(); cnt = (C.c_long * 5)()
         self._chk(self.lib.lise_profile_read(self._h, ms, cnt), "lise_profile_read")
         return {n: (ms[i], cnt[i]) for i, n in enumerate(self.PROFILE_CLASSES)}
+
+    def line_operator(self):
+        return self.lib.lise_line_operator(self._h).decode()
 
     def launch_count(self):
         return int(self.lib.lise_launch_count(self._h))
