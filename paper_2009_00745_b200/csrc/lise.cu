@@ -7,6 +7,7 @@
 // densities of the new state) -> k_dens_x (x densities of the new state).
 #include "common.cuh"
 #include "state_kernels.cuh"
+#include "plane_kernels.cuh"
 #include "grid_kernels.cuh"
 #include "peak_kernels.cuh"
 #include <new>
@@ -23,6 +24,7 @@ struct KernSet {
     UKern u[4];
     DKern d_x;
     const char* name;
+    int ncomp_yz, ncomp_xz;
 };
 struct lise_ctx {
     Lattice L;
@@ -169,21 +171,49 @@ static KernSet make_set(const char* name)
     k.name = name;
     return k;
 }
-// DMMA line operators exist for these (nx; ny, nz) combinations (every lattice of BASELINE.json's configs
-// except the 12^3 one of config 0 ... which is listed too); anything else runs the generic DFMA kernels.
+// shared-memory footprints of the v3 plane kernels (bytes), see plane_kernels.cuh
+static constexpr size_t v3_smem_happly_yz(int ny, int nz, int ncomp)
+{
+    return 16 * (size_t)(2 * ny + 2 * nz + 4 * ny * nz + 2 * ncomp * ny * nz) + 8 * (size_t)(ny * nz);
+}
+static constexpr size_t v3_smem_happly_xz(int nx, int nz, int ncomp)
+{
+    return 16 * (size_t)(2 * nx + 2 * nx * nz + 2 * ncomp * nx * nz) + 8 * (size_t)(nx * nz + 64);
+}
+static constexpr size_t v3_smem_update(int ny, int nz) { return 16 * (size_t)(2 * ny + 2 * nz + 2 * ny * nz) + 8 * (size_t)(LISE_NACC * ny * nz + 8); }
+static constexpr size_t v3_smem_dens_x(int nx, int nz) { return 16 * (size_t)(2 * nx + 2 * nx * nz) + 8 * (size_t)(LISE_NACC * nx * nz); }
+static constexpr size_t SMEM_LIMIT = 227 * 1024;
+
+template <int NX, int NY, int NZ>
+static KernSet make_v3_set()
+{
+    constexpr int CYZ = (v3_smem_happly_yz(NY, NZ, 4) <= SMEM_LIMIT) ? 4 : 2;
+    constexpr int CXZ = (v3_smem_happly_xz(NX, NZ, 4) <= SMEM_LIMIT) ? 4 : 2;
+    KernSet k;
+    k.h_yz = k3_happly_yz<NY, NZ, CYZ>; k.h_xz = k3_happly_xz<NX, CXZ>;
+    k.u[0] = k3_update_yz<0, NY, NZ>; k.u[1] = k3_update_yz<1, NY, NZ>; k.u[2] = k3_update_yz<2, NY, NZ>; k.u[3] = k3_update_yz<3, NY, NZ>;
+    k.d_x = k3_dens_x<NX>;
+    k.name = "dmma";
+    k.ncomp_yz = CYZ; k.ncomp_xz = CXZ;
+    return k;
+}
+// The DMMA plane kernels are instantiated for these lattices (nx, ny, nz): every lattice of BASELINE.json's
+// configs, the paper's 24^2 x 48, and two small non-cubic test shapes; every edge a multiple of 4 and the
+// planes small enough for shared memory.  Anything else runs the generic DFMA kernels.
 #define LISE_MMA_SHAPES(X) \
-    X(8, 8, 8) X(12, 12, 12) X(16, 16, 16) X(20, 20, 20) X(24, 24, 24) X(32, 32, 32) X(40, 40, 40) X(48, 48, 48) X(64, 64, 64) \
-    X(24, 24, 48) X(24, 24, 64) X(12, 8, 16) X(16, 12, 8) X(32, 32, 64)
+    X(8, 8, 8) X(12, 12, 12) X(16, 16, 16) X(20, 20, 20) X(24, 24, 24) X(32, 32, 32) X(40, 40, 40) \
+    X(24, 24, 48) X(24, 24, 64) X(12, 8, 16) X(16, 12, 8)
 static bool pick_kernels(int nx, int ny, int nz, int R, bool want_mma, KernSet* out)
 {
     if (want_mma) {
-#define X(a, b, c_) if (nx == a && ny == b && nz == c_) { *out = make_set<MmaLines<b, c_>, MmaLines<a, 0>>("dmma"); return true; }
+#define X(a, b, c_) if (nx == a && ny == b && nz == c_) { *out = make_v3_set<a, b, c_>(); return true; }
         LISE_MMA_SHAPES(X)
 #undef X
     }
     if (R == 8) *out = make_set<DenseLines<8>, DenseLines<8>>("dense");
     else if (R == 4) *out = make_set<DenseLines<4>, DenseLines<4>>("dense");
     else *out = make_set<DenseLines<2>, DenseLines<2>>("dense");
+    out->ncomp_yz = out->ncomp_xz = 2;
     return false;
 }
 
@@ -494,17 +524,24 @@ static int ctx_init(lise_ctx* c)
     c->mma = pick_kernels(L.nx, L.ny, L.nz, c->R, want_mma, &c->ks) ? 1 : 0;
     const int ld = L.nz + 1;
     const int n1[2] = {L.ny, L.nx};
-    for (int k = 0; k < 2; ++k) {
-        const int npts = n1[k] * L.nz;
-        int t = c->mma ? 256 : ((2 * npts / c->R + 31) / 32) * 32;
-        if (c->mma && npts <= 256) t = 128;
-        if (t > 512) t = 512;
-        if (t < 64) t = 64;
-        c->thr[k] = t;
-        c->smem_h[k] = sizeof(double2) * (size_t)(2 * (n1[k] + L.nz) + 8 * n1[k] * ld) + 64 * sizeof(double);
+    if (c->mma) {
+        c->thr[0] = c->thr[1] = 256;
+        c->smem_h[0] = v3_smem_happly_yz(L.ny, L.nz, c->ks.ncomp_yz);
+        c->smem_h[1] = v3_smem_happly_xz(L.nx, L.nz, c->ks.ncomp_xz);
+        c->smem_u = v3_smem_update(L.ny, L.nz);
+        c->smem_d = v3_smem_dens_x(L.nx, L.nz);
+    } else {
+        for (int k = 0; k < 2; ++k) {
+            const int npts = n1[k] * L.nz;
+            int t = ((2 * npts / c->R + 31) / 32) * 32;
+            if (t > 512) t = 512;
+            if (t < 64) t = 64;
+            c->thr[k] = t;
+            c->smem_h[k] = sizeof(double2) * (size_t)(2 * (n1[k] + L.nz) + 8 * n1[k] * ld) + 64 * sizeof(double);
+        }
+        c->smem_u = sizeof(double2) * (size_t)(2 * (L.ny + L.nz) + 6 * L.ny * ld) + 64 * sizeof(double);
+        c->smem_d = sizeof(double2) * (size_t)(2 * L.nx + 6 * L.nx * ld);
     }
-    c->smem_u = sizeof(double2) * (size_t)(2 * (L.ny + L.nz) + 6 * L.ny * ld) + 64 * sizeof(double);
-    c->smem_d = sizeof(double2) * (size_t)(2 * L.nx + 6 * L.nx * ld);
     const size_t lim = 227 * 1024;
     if (c->smem_h[0] > lim || c->smem_h[1] > lim || c->smem_u > lim || c->smem_d > lim) {
         snprintf(c->err, sizeof(c->err), "lattice planes too large for shared memory (%zu bytes needed, %zu available)",
@@ -512,8 +549,17 @@ static int ctx_init(lise_ctx* c)
         return LISE_EUNSUPPORTED;
     }
     TRY(set_attrs(c));
-    int minp = L.nx < L.ny ? L.nx : L.ny;
-    c->G = (2 * 148 + minp - 1) / minp;
+    int nsm = 148;
+    { int dev = 0; if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev); if (nsm < 1) nsm = 148; }
+    if (c->mma) {
+        // plane-owner CTAs, one per SM: as many state groups as fit the SM count
+        const int maxp = L.nx > L.ny ? L.nx : L.ny;
+        c->G = nsm / maxp;
+    } else {
+        const int minp = L.nx < L.ny ? L.nx : L.ny;
+        c->G = (2 * nsm + minp - 1) / minp;
+    }
+    if (const char* e = getenv("LISE_G")) { int g = atoi(e); if (g > 0) c->G = g; }
     if (c->G > LISE_MAXG) c->G = LISE_MAXG;
     if (c->G < 1) c->G = 1;
     c->chunk = default_chunk(c);
