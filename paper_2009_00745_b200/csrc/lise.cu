@@ -7,7 +7,7 @@
 // densities of the new state) -> k_dens_x (x densities of the new state).
 #include "common.cuh"
 #include "state_kernels.cuh"
-#include "plane_kernels.cuh"
+#include "plane4_kernels.cuh"
 #include "grid_kernels.cuh"
 #include "peak_kernels.cuh"
 #include <new>
@@ -24,7 +24,9 @@ struct KernSet {
     UKern u[4];
     DKern d_x;
     const char* name;
-    int ncomp_yz, ncomp_xz;
+    int thr_h[2], thr_u, thr_d;            // threads per CTA: happly yz / xz, update, dens_x
+    size_t smem_h[2], smem_u, smem_d;      // dynamic shared memory, bytes (0 = filled by ctx_init for the generic path)
+    int ups_xz;                            // eta partial sums per state = ups_xz * ny
 };
 struct lise_ctx {
     Lattice L;
@@ -49,9 +51,8 @@ struct lise_ctx {
     cplx *tw, *cA1, *cA2, *cA3;
     double* ebuf; int eblocks;
     cplx* ovl;
-    int R, thr[2], mma;
+    int R, mma;
     KernSet ks;
-    size_t smem_h[2], smem_u, smem_d;
     int have[2], pot_valid;
     long step; double time;
     long launches; long long bytes;
@@ -171,30 +172,49 @@ static KernSet make_set(const char* name)
     k.name = name;
     return k;
 }
-// shared-memory footprints of the v3 plane kernels (bytes), see plane_kernels.cuh
-static constexpr size_t v3_smem_happly_yz(int ny, int nz, int ncomp)
-{
-    return 16 * (size_t)(2 * ny + 2 * nz + 4 * ny * nz + 2 * ncomp * ny * nz) + 8 * (size_t)(ny * nz);
-}
-static constexpr size_t v3_smem_happly_xz(int nx, int nz, int ncomp)
-{
-    return 16 * (size_t)(2 * nx + 2 * nx * nz + 2 * ncomp * nx * nz) + 8 * (size_t)(nx * nz + 64);
-}
-static constexpr size_t v3_smem_update(int ny, int nz) { return 16 * (size_t)(2 * ny + 2 * nz + 2 * ny * nz) + 8 * (size_t)(LISE_NACC * ny * nz + 8); }
-static constexpr size_t v3_smem_dens_x(int nx, int nz) { return 16 * (size_t)(2 * nx + 2 * nx * nz) + 8 * (size_t)(LISE_NACC * nx * nz); }
+// ---- v4 plane kernels: compile-time choice of unit size (NCOMP), prefetch depth (NBUF), warps, staging ----
 static constexpr size_t SMEM_LIMIT = 227 * 1024;
+static constexpr size_t v4_smem_happly_yz(int ny, int nz, int ncomp, int nbuf, bool vstage)
+{
+    return 16 * (size_t)(2 * ny + 2 * nz) + 16 * (size_t)(ny * ldpad(nz)) * ncomp * (nbuf + 1)
+         + 8 * (size_t)(ny * ldpad(nz)) * (6 + (vstage ? 6 : 0));
+}
+static constexpr size_t v4_smem_happly_xz(int nx, int nz, int ncomp, int nbuf)
+{
+    return 16 * (size_t)(2 * nx) + 16 * (size_t)(nx * ldpad(nz)) * ncomp * 2 * nbuf + 8 * (size_t)(nx * ldpad(nz)) * 4 + 8 * 64;
+}
+static constexpr size_t v4_smem_update(int ny, int nz) { return 16 * (size_t)(2 * ny + 2 * nz) + 16 * (size_t)(2 * ny * ldpad(nz)); }
+static constexpr size_t v4_smem_dens_x(int nx, int nz) { return 16 * (size_t)(2 * nx) + 16 * (size_t)(2 * nx * ldpad(nz)); }
+static constexpr int imin(int a, int b) { return a < b ? a : b; }
+static constexpr int imax(int a, int b) { return a > b ? a : b; }
+// warps of an H-apply CTA: one strip task per warp if possible; long lines need more registers per thread
+static constexpr int v4_warps_h(int tasks, int nline) { return imin(tasks, nline >= 32 ? 8 : 12); }
 
 template <int NX, int NY, int NZ>
-static KernSet make_v3_set()
+static KernSet make_v4_set()
 {
-    constexpr int CYZ = (v3_smem_happly_yz(NY, NZ, 4) <= SMEM_LIMIT) ? 4 : 2;
-    constexpr int CXZ = (v3_smem_happly_xz(NX, NZ, 4) <= SMEM_LIMIT) ? 4 : 2;
+    // yz: prefer whole states with prefetch, then 2-spinors with prefetch, then 2-spinors without
+    constexpr int CYZ = (v4_smem_happly_yz(NY, NZ, 4, 2, false) <= SMEM_LIMIT) ? 4 : 2;
+    constexpr int BYZ = (v4_smem_happly_yz(NY, NZ, CYZ, 2, false) <= SMEM_LIMIT) ? 2 : 1;
+    constexpr bool VST = v4_smem_happly_yz(NY, NZ, CYZ, BYZ, true) <= SMEM_LIMIT;
+    constexpr int WYZ = v4_warps_h((CYZ / 2) * imax(NY, NZ) / 4, imax(NY, NZ));
+    constexpr int CXZ = (v4_smem_happly_xz(NX, NZ, 4, 2) <= SMEM_LIMIT) ? 4 : 2;
+    constexpr int BXZ = (v4_smem_happly_xz(NX, NZ, CXZ, 2) <= SMEM_LIMIT) ? 2 : 1;
+    constexpr int WXZ = v4_warps_h((CXZ / 2) * NZ / 4, NX);
+    constexpr int WU = imin(2 * imax(NY, NZ) / 4, imax(NY, NZ) >= 32 ? 8 : 12);
+    constexpr int WD = imin(2 * NZ / 4, imax(NX, NZ) >= 32 ? 8 : 12);
+    static_assert(v4_smem_happly_yz(NY, NZ, CYZ, BYZ, VST) <= SMEM_LIMIT, "yz plane too large");
+    static_assert(v4_smem_happly_xz(NX, NZ, CXZ, BXZ) <= SMEM_LIMIT, "xz plane too large");
     KernSet k;
-    k.h_yz = k3_happly_yz<NY, NZ, CYZ>; k.h_xz = k3_happly_xz<NX, CXZ>;
-    k.u[0] = k3_update_yz<0, NY, NZ>; k.u[1] = k3_update_yz<1, NY, NZ>; k.u[2] = k3_update_yz<2, NY, NZ>; k.u[3] = k3_update_yz<3, NY, NZ>;
-    k.d_x = k3_dens_x<NX>;
+    k.h_yz = k4_happly_yz<NY, NZ, CYZ, BYZ, WYZ, VST>; k.h_xz = k4_happly_xz<NX, NZ, CXZ, BXZ, WXZ>;
+    k.u[0] = k4_update_yz<0, NY, NZ, WU>; k.u[1] = k4_update_yz<1, NY, NZ, WU>;
+    k.u[2] = k4_update_yz<2, NY, NZ, WU>; k.u[3] = k4_update_yz<3, NY, NZ, WU>;
+    k.d_x = k4_dens_x<NX, NZ, WD>;
     k.name = "dmma";
-    k.ncomp_yz = CYZ; k.ncomp_xz = CXZ;
+    k.thr_h[0] = 32 * WYZ; k.thr_h[1] = 32 * WXZ; k.thr_u = 32 * WU; k.thr_d = 32 * WD;
+    k.smem_h[0] = v4_smem_happly_yz(NY, NZ, CYZ, BYZ, VST); k.smem_h[1] = v4_smem_happly_xz(NX, NZ, CXZ, BXZ);
+    k.smem_u = v4_smem_update(NY, NZ); k.smem_d = v4_smem_dens_x(NX, NZ);
+    k.ups_xz = 4 / CXZ;
     return k;
 }
 // The DMMA plane kernels are instantiated for these lattices (nx, ny, nz): every lattice of BASELINE.json's
@@ -206,14 +226,16 @@ static KernSet make_v3_set()
 static bool pick_kernels(int nx, int ny, int nz, int R, bool want_mma, KernSet* out)
 {
     if (want_mma) {
-#define X(a, b, c_) if (nx == a && ny == b && nz == c_) { *out = make_v3_set<a, b, c_>(); return true; }
+#define X(a, b, c_) if (nx == a && ny == b && nz == c_) { *out = make_v4_set<a, b, c_>(); return true; }
         LISE_MMA_SHAPES(X)
 #undef X
     }
     if (R == 8) *out = make_set<DenseLines<8>, DenseLines<8>>("dense");
     else if (R == 4) *out = make_set<DenseLines<4>, DenseLines<4>>("dense");
     else *out = make_set<DenseLines<2>, DenseLines<2>>("dense");
-    out->ncomp_yz = out->ncomp_xz = 2;
+    out->thr_h[0] = out->thr_h[1] = out->thr_u = out->thr_d = 0;
+    out->smem_h[0] = out->smem_h[1] = out->smem_u = out->smem_d = 0;
+    out->ups_xz = 1;
     return false;
 }
 
@@ -222,7 +244,7 @@ static int launch_happly(lise_ctx* c, const HArgs& a)
 {
     dim3 grid(KIND == 0 ? c->L.nx : c->L.ny, c->G);
     prof_begin(c, KIND == 0 ? PC_HAPPLY_YZ : PC_HAPPLY_XZ);
-    (KIND == 0 ? c->ks.h_yz : c->ks.h_xz)<<<grid, c->thr[KIND], c->smem_h[KIND], c->stream>>>(a);
+    (KIND == 0 ? c->ks.h_yz : c->ks.h_xz)<<<grid, c->ks.thr_h[KIND], c->ks.smem_h[KIND], c->stream>>>(a);
     prof_end(c);
     CKL();
     return LISE_OK;
@@ -232,7 +254,7 @@ static int launch_update(lise_ctx* c, const UArgs& a)
 {
     dim3 grid(c->L.nx, c->G);
     prof_begin(c, PC_UPDATE);
-    c->ks.u[MODE]<<<grid, c->thr[0], c->smem_u, c->stream>>>(a);
+    c->ks.u[MODE]<<<grid, c->ks.thr_u, c->ks.smem_u, c->stream>>>(a);
     prof_end(c);
     CKL();
     return LISE_OK;
@@ -241,17 +263,17 @@ static int launch_dens_x(lise_ctx* c, const DArgs& a)
 {
     dim3 grid(c->L.ny, c->G);
     prof_begin(c, PC_DENS_X);
-    c->ks.d_x<<<grid, c->thr[1], c->smem_d, c->stream>>>(a);
+    c->ks.d_x<<<grid, c->ks.thr_d, c->ks.smem_d, c->stream>>>(a);
     prof_end(c);
     CKL();
     return LISE_OK;
 }
 static int set_attrs(lise_ctx* c)
 {
-    CK(cudaFuncSetAttribute(c->ks.h_yz, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_h[0]));
-    CK(cudaFuncSetAttribute(c->ks.h_xz, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_h[1]));
-    for (int m = 0; m < 4; ++m) CK(cudaFuncSetAttribute(c->ks.u[m], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_u));
-    CK(cudaFuncSetAttribute(c->ks.d_x, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_d));
+    CK(cudaFuncSetAttribute(c->ks.h_yz, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->ks.smem_h[0]));
+    CK(cudaFuncSetAttribute(c->ks.h_xz, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->ks.smem_h[1]));
+    for (int m = 0; m < 4; ++m) CK(cudaFuncSetAttribute(c->ks.u[m], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->ks.smem_u));
+    CK(cudaFuncSetAttribute(c->ks.d_x, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->ks.smem_d));
     return LISE_OK;
 }
 
@@ -276,7 +298,7 @@ static UArgs make_uargs(lise_ctx* c, int q, size_t off, int ns)
     u.sE = S(c, q, RE) + off; u.sF = S(c, q, RF) + off; u.sG = S(c, q, RG) + off;
     u.Z = nullptr; u.eta_part = c->eta_part; u.eta_fix = c->eta_fix; u.part = c->part[q];
     fill_common(c, u.ctab);
-    u.dt = c->dt; u.hbarc = c->par.hbarc; u.ns = ns; u.G = c->G; u.order = 0; u.remove_phase = c->par.remove_phase;
+    u.neta = c->ks.ups_xz * c->L.ny; u.dt = c->dt; u.hbarc = c->par.hbarc; u.ns = ns; u.G = c->G; u.order = 0; u.remove_phase = c->par.remove_phase;
     u.write_f = 1;
     return u;
 }
@@ -522,30 +544,25 @@ static int ctx_init(lise_ctx* c)
     bool want_mma = true;
     if (const char* e = getenv("LISE_LINE_OP")) want_mma = (strcmp(e, "dense") != 0);
     c->mma = pick_kernels(L.nx, L.ny, L.nz, c->R, want_mma, &c->ks) ? 1 : 0;
-    const int ld = L.nz + 1;
-    const int n1[2] = {L.ny, L.nx};
-    if (c->mma) {
-        c->thr[0] = c->thr[1] = 256;
-        c->smem_h[0] = v3_smem_happly_yz(L.ny, L.nz, c->ks.ncomp_yz);
-        c->smem_h[1] = v3_smem_happly_xz(L.nx, L.nz, c->ks.ncomp_xz);
-        c->smem_u = v3_smem_update(L.ny, L.nz);
-        c->smem_d = v3_smem_dens_x(L.nx, L.nz);
-    } else {
+    if (!c->mma) {
+        const int ld = L.nz + 1;
+        const int n1[2] = {L.ny, L.nx};
         for (int k = 0; k < 2; ++k) {
             const int npts = n1[k] * L.nz;
             int t = ((2 * npts / c->R + 31) / 32) * 32;
             if (t > 512) t = 512;
             if (t < 64) t = 64;
-            c->thr[k] = t;
-            c->smem_h[k] = sizeof(double2) * (size_t)(2 * (n1[k] + L.nz) + 8 * n1[k] * ld) + 64 * sizeof(double);
+            c->ks.thr_h[k] = t;
+            c->ks.smem_h[k] = sizeof(double2) * (size_t)(2 * (n1[k] + L.nz) + 8 * n1[k] * ld) + 64 * sizeof(double);
         }
-        c->smem_u = sizeof(double2) * (size_t)(2 * (L.ny + L.nz) + 6 * L.ny * ld) + 64 * sizeof(double);
-        c->smem_d = sizeof(double2) * (size_t)(2 * L.nx + 6 * L.nx * ld);
+        c->ks.thr_u = c->ks.thr_h[0]; c->ks.thr_d = c->ks.thr_h[1];
+        c->ks.smem_u = sizeof(double2) * (size_t)(2 * (L.ny + L.nz) + 6 * L.ny * ld) + 64 * sizeof(double);
+        c->ks.smem_d = sizeof(double2) * (size_t)(2 * L.nx + 6 * L.nx * ld);
     }
     const size_t lim = 227 * 1024;
-    if (c->smem_h[0] > lim || c->smem_h[1] > lim || c->smem_u > lim || c->smem_d > lim) {
+    if (c->ks.smem_h[0] > lim || c->ks.smem_h[1] > lim || c->ks.smem_u > lim || c->ks.smem_d > lim) {
         snprintf(c->err, sizeof(c->err), "lattice planes too large for shared memory (%zu bytes needed, %zu available)",
-                 c->smem_h[0] > c->smem_h[1] ? c->smem_h[0] : c->smem_h[1], lim);
+                 c->ks.smem_h[0] > c->ks.smem_h[1] ? c->ks.smem_h[0] : c->ks.smem_h[1], lim);
         return LISE_EUNSUPPORTED;
     }
     TRY(set_attrs(c));
@@ -582,7 +599,7 @@ static int ctx_init(lise_ctx* c)
     c->wcap = nmax < 512 ? (nmax > 0 ? nmax : 1) : 512;     // largest chunk lise_set_chunk accepts
     if (c->wcap < c->chunk) c->wcap = c->chunk;
     DM(c->W, (size_t)c->wcap * 4 * nx);
-    DM(c->eta_part, (size_t)c->wcap * L.ny);
+    DM(c->eta_part, (size_t)c->wcap * L.ny * 2);
     DM(c->eta_fix, (size_t)c->wcap);
     for (int q = 0; q < 2; ++q) {
         DM(c->part[q], (size_t)LISE_MAXG * LISE_NACC * nx);

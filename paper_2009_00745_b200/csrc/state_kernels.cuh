@@ -442,6 +442,7 @@ struct UArgs {
     const double2* ctab[3];
     double dt, hbarc;
     int ns, G, order, remove_phase, write_f;
+    int neta;                                  // eta partial sums per state (v4 kernels; the generic ones use L.ny)
 };
 
 template <int MODE, class LO>
