@@ -99,28 +99,36 @@ def make_shard(cfg, q, nwf_total, first, count, seed, device):
     return inputs.make_block(cfg, q, nwf_total, first, count, seed, device)
 
 
-# per-kernel-class algorithmic traffic in units of one state array S = 64 Nxyz bytes per state processed,
-# and fp64 instructions (DFMA-pipe issue slots) per lattice point per state processed (kernel table)
+# per-kernel-class algorithmic traffic in units of one state array S = 64 Nxyz bytes per state processed, and
+# fp64-pipe work (FMA-equivalents: 256 per DMMA m8n8k4, 1 per DFMA) per lattice point per state processed
+# (kernel table).  Block-diagonalised circulant: a line of N = 8 R points costs
+# dmma(N) = 2 (real blocks) + 8 (conjugate pairs) tiles per 8 real columns and operator application.
+def dmma_tiles(n):
+    if n % 8 == 0 and 16 <= n <= 64:
+        r = n // 8
+        nreal = 1 + (1 if r % 2 == 0 else 0)
+        return 2 * nreal + 8 * ((r - 1) // 2)
+    return ((n + 7) // 8) * (n // 4)                               # plain circulant
+
+
+def line_fma_per_point(n):
+    """DMMA FMAs per complex lattice point for ONE operator application along a line of n points."""
+    return dmma_tiles(n) * 256.0 / (4.0 * n)                       # a tile covers 4 complex lines (8 real columns)
+
+
 def class_model(shape, line_op):
     nx, ny, nz = shape
     if line_op == "dense":
-        # circulant sums: 8 N pipe slots per point per component for each of the two line passes of an axis
-        happly_yz = 4 * 16 * (ny + nz) + 4 * 60
-        happly_xz = 4 * 16 * nx + 4 * 30
-        dens_yz = 2 * 8 * (ny + nz) + 60
-        dens_x = 2 * 8 * nx + 30
+        fx, fy, fz = (2.0 * n for n in (nx, ny, nz))                 # DFMA circulant sums: 2 N per complex point
     else:
-        def fft(n):     # ~ pipe slots per point of one length-n transform (radix-4/2/3/5 mix), DESIGN.md
-            return 2.8 * math.log2(n)
-        happly_yz = 4 * 6 * (fft(ny) + fft(nz)) + 4 * 60
-        happly_xz = 4 * 6 * fft(nx) + 4 * 30
-        dens_yz = 2 * 3 * (fft(ny) + fft(nz)) + 60
-        dens_x = 2 * 3 * fft(nx) + 30
+        fx, fy, fz = (line_fma_per_point(n) for n in (nx, ny, nz))
+    pw_h = 50.0                                                    # pointwise FMAs per point, component and axis (B, M products, real DFT)
     return {
-        "happly_yz": dict(S=2.0, slots=happly_yz),                 # read X, write W
-        "happly_xz": dict(S=3.0, slots=happly_xz),                 # read X, W; write W
-        "update_yz": dict(S=8.5, slots=dens_yz + 40),              # evaluation 1: 11 S, evaluation 2: 6 S -> mean 8.5
-        "dens_x": dict(S=0.5, slots=dens_x),                       # read v_up, v_dn of the new state
+        "happly_yz": dict(S=2.0, slots=4 * (4 * (fy + fz) + 2 * pw_h) + 4 * 12),   # read X, write W
+        "happly_xz": dict(S=3.0, slots=4 * (4 * fx + pw_h)),                       # read X, W; write W
+        "update": dict(S=8.5, slots=40.0),                         # evaluation 1: 7 + 4 S, evaluation 2: 4 + 2 S -> mean 8.5
+        "dens_yz": dict(S=0.75, slots=2 * (2 * (fy + fz) + 20) + 20),              # read v_up, v_dn, u_up of the new state
+        "dens_x": dict(S=0.5, slots=2 * (2 * fx + 10)),            # read v_up, v_dn of the new state
         "grid": dict(S=0.0, slots=0.0),
     }
 

@@ -79,6 +79,11 @@ int lise_set_stream(lise_ctx *ctx, void *cuda_stream);       /* cudaStream_t own
 int lise_set_dt(lise_ctx *ctx, double dt);
 /* Number of states processed per kernel launch (L2-resident batching of intermediates); <= 0 restores the default. */
 int lise_set_chunk(lise_ctx *ctx, int nstates);
+/* Tensor-core kernels only: enable (default, or LISE_OVERLAP=0/1 in the environment) or disable running the
+ * HBM-bound ABM update kernels on an internal second stream concurrently with the DMMA-bound kernels of the
+ * neighbouring chunks.  Results are bit-identical either way.  All work is ordered back into the context's
+ * stream before lise_step returns. */
+int lise_set_overlap(lise_ctx *ctx, int enable);
 
 /* Copies nwf_q states in (device pointer, layout above), accumulates their densities and resets the
  * multistep history, step counter and time. */
@@ -131,8 +136,11 @@ int lise_observables(lise_ctx *ctx, lise_observables_t *host_out);
  * (and around each grid-only phase); lise_profile_read synchronises and returns the summed
  * milliseconds and launch counts per class, then clears the record.  Classes:
  *   0 H-apply on yz-planes (y and z lines), 1 H-apply on xz-planes (x lines, eta),
- *   2 ABM update + y/z density pass, 3 x density pass, 4 grid-only phase (reduction, potentials, Coulomb).
- * ms and counts are HOST arrays of 5 entries. */
+ *   2 ABM update (generic kernels: + y/z density pass), 3 x density pass, 4 grid-only phase (reduction,
+ *   potentials, Coulomb), 5 pointwise + y/z density pass (tensor-core kernels only).
+ * Each pair is recorded on the stream its kernel is launched on (the update kernels run on an internal second
+ * stream when overlap is on, see lise_set_overlap), so class times may overlap in wall time.
+ * ms and counts are HOST arrays of 6 entries. */
 int lise_profile(lise_ctx *ctx, int enable);
 int lise_profile_read(lise_ctx *ctx, double *ms, long *counts);
 

@@ -6,7 +6,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "liblise.so")
 SOURCES = ["lise.cu"]
-HEADERS = ["common.cuh", "state_kernels.cuh", "grid_kernels.cuh", "plane4_kernels.cuh", "peak_kernels.cuh", os.path.join("..", "..", "include", "lise.h")]
+HEADERS = ["common.cuh", "state_kernels.cuh", "grid_kernels.cuh", "plane_common.cuh", "split_lineop.cuh", "plane5_kernels.cuh", "peak_kernels.cuh", os.path.join("..", "..", "include", "lise.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]
 

@@ -7,7 +7,7 @@
 // densities of the new state) -> k_dens_x (x densities of the new state).
 #include "common.cuh"
 #include "state_kernels.cuh"
-#include "plane4_kernels.cuh"
+#include "plane5_kernels.cuh"
 #include "grid_kernels.cuh"
 #include "peak_kernels.cuh"
 #include <new>
@@ -22,10 +22,11 @@ typedef void (*DKern)(DArgs);
 struct KernSet {
     HKern h_yz, h_xz;
     UKern u[4];
-    DKern d_x;
+    DKern d_x, d_yz;                       // d_yz: plane5 kernels only (the generic update kernel carries the y/z densities)
     const char* name;
-    int thr_h[2], thr_u, thr_d;            // threads per CTA: happly yz / xz, update, dens_x
-    size_t smem_h[2], smem_u, smem_d;      // dynamic shared memory, bytes (0 = filled by ctx_init for the generic path)
+    int v5;                                // plane5 kernel set: pure-streaming update + separate density kernels
+    int thr_h[2], thr_u, thr_d, thr_dyz;   // threads per CTA: happly yz / xz, update, dens_x, dens_yz
+    size_t smem_h[2], smem_u, smem_d, smem_dyz;   // dynamic shared memory, bytes (0 = filled by ctx_init for the generic path)
     int ups_xz;                            // eta partial sums per state = ups_xz * ny
 };
 struct lise_ctx {
@@ -37,11 +38,15 @@ struct lise_ctx {
     PhysConst pc;
     cudaStream_t stream;
     double2* ctab[3];
+    double* stab[3];                        // block-diagonalised line-operator tables (split_lineop.cuh)
+    cudaStream_t stream2;                   // the HBM-bound update kernels run here, overlapping the DMMA kernels
+    cudaEvent_t ev_h[2], ev_u[2];
+    int overlap;
     cplx* slot[2][LISE_NSLOT];
     int role[LISE_NSLOT];
-    cplx* W;
+    cplx* W;                                // [2][wcap] states: H-apply output, double-buffered across chunks
     int chunk, wcap;
-    double *eta_part, *eta_fix;
+    double *eta_part, *eta_fix;             // eta_part: [2][wcap][neta]
     int G;
     double *part[2], *acc[2], *acc0[2], *dens[2], *pot[2], *geff[2];
     double *gtmp, *phi;
@@ -65,22 +70,24 @@ struct lise_ctx {
     char err[256];
 };
 
-enum { PC_HAPPLY_YZ = 0, PC_HAPPLY_XZ, PC_UPDATE, PC_DENS_X, PC_GRID, PC_NCLASS };
+enum { PC_HAPPLY_YZ = 0, PC_HAPPLY_XZ, PC_UPDATE, PC_DENS_X, PC_GRID, PC_DENS_YZ, PC_NCLASS };
 
-static void prof_begin(lise_ctx* c, int cls)
+static void prof_begin(lise_ctx* c, int cls, cudaStream_t st = nullptr)
 {
     if (!c->prof) return;
+    if (!st) st = c->stream;
     if ((size_t)(2 * c->prof_n + 2) > c->prof_ev->size()) {
         cudaEvent_t a, b; cudaEventCreate(&a); cudaEventCreate(&b);
         c->prof_ev->push_back(a); c->prof_ev->push_back(b); c->prof_cls->push_back(cls);
     }
     (*c->prof_cls)[c->prof_n] = cls;
-    cudaEventRecord((*c->prof_ev)[2 * c->prof_n], c->stream);
+    cudaEventRecord((*c->prof_ev)[2 * c->prof_n], st);
 }
-static void prof_end(lise_ctx* c)
+static void prof_end(lise_ctx* c, cudaStream_t st = nullptr)
 {
     if (!c->prof) return;
-    cudaEventRecord((*c->prof_ev)[2 * c->prof_n + 1], c->stream);
+    if (!st) st = c->stream;
+    cudaEventRecord((*c->prof_ev)[2 * c->prof_n + 1], st);
     c->prof_n++;
 }
 
@@ -131,6 +138,66 @@ static void host_ctab(int N, double a, std::vector<double2>& t)
     }
 }
 
+// ---- block-diagonalised tables of split_lineop.cuh: tab[((op * J + j) * 2 + pq) * ND + d + H - 1] ----
+struct LOpDims { int N, H, R, J, NTH, NKH, ND, TABSZ; };
+static LOpDims lop_dims(int N)
+{
+    LOpDims d;
+    d.N = N; d.H = (N % 8 == 0 && N >= 16 && N / 8 <= LISE_RMAX) ? 8 : N;
+    d.R = N / d.H; d.J = d.R / 2 + 1; d.NTH = (d.H + 7) / 8; d.NKH = d.H / 4;
+    d.ND = d.H + 8 * d.NTH - 1; d.TABSZ = 2 * d.J * 2 * d.ND;
+    return d;
+}
+static void host_stab(int N, double a, std::vector<double>& tab)
+{
+    std::vector<double2> ct;
+    host_ctab(N, a, ct);                       // ct[N + d] = (c1, c2)[d mod N]
+    const LOpDims D = lop_dims(N);
+    const long double pi = 3.14159265358979323846264338327950288L;
+    tab.assign(D.TABSZ, 0.0);
+    for (int op = 0; op < 2; ++op)
+        for (int j = 0; j < D.J; ++j) {
+            const long double w = (j == 0 || 2 * j == D.R) ? 1.0L : 2.0L;
+            for (int d = -(D.H - 1); d < D.H; ++d) {           // d >= H: padding rows, left 0
+                long double P = 0.0L, Q = 0.0L;
+                for (int p = 0; p < D.R; ++p) {
+                    const int k = (((d + D.H * p) % N) + N) % N;
+                    const long double cv = op ? ct[N + k].y : ct[N + k].x;
+                    const int jp = (j * p) % D.R;
+                    const long double th = 2.0L * pi * jp / D.R;
+                    const long double co = (4 * jp == D.R || 4 * jp == 3 * D.R) ? 0.0L : cosl(th);
+                    const long double si = (jp == 0 || 2 * jp == D.R) ? 0.0L : sinl(th);
+                    P += co * cv; Q += si * cv;
+                }
+                tab[((op * D.J + j) * 2 + 0) * D.ND + d + D.H - 1] = (double)(w / D.R * P);
+                tab[((op * D.J + j) * 2 + 1) * D.ND + d + D.H - 1] = (double)(w / D.R * Q);
+            }
+        }
+}
+// generic real-DFT coefficients in constant memory: c_rdft[R][q][m] (spectral order of split_lineop.cuh)
+static int upload_rdft()
+{
+    static double h[LISE_RMAX + 1][LISE_RMAX][LISE_RMAX];
+    const long double pi = 3.14159265358979323846264338327950288L;
+    memset(h, 0, sizeof(h));
+    for (int R = 1; R <= LISE_RMAX; ++R)
+        for (int q = 0; q < R; ++q) {
+            int j; bool sn;
+            if (q == 0) { j = 0; sn = false; }
+            else if (R % 2 == 0 && q == R - 1) { j = R / 2; sn = false; }
+            else { j = (q + 1) / 2; sn = (q % 2 == 0); }
+            for (int m = 0; m < R; ++m) {
+                const int jm = (j * m) % R;
+                const long double th = 2.0L * pi * jm / R;
+                long double v;
+                if (sn) v = (jm == 0 || 2 * jm == R) ? 0.0L : sinl(th);
+                else    v = (4 * jm == R || 4 * jm == 3 * R) ? 0.0L : cosl(th);
+                h[R][q][m] = (double)v;
+            }
+        }
+    return cudaMemcpyToSymbol(c_rdft, h, sizeof(h)) == cudaSuccess ? LISE_OK : LISE_ECUDA;
+}
+
 static void set_physconst(lise_ctx* c)
 {
     const lise_params& p = c->par;
@@ -168,52 +235,57 @@ static KernSet make_set(const char* name)
     KernSet k;
     k.h_yz = k_happly<0, LOYZ>; k.h_xz = k_happly<1, LOXZ>;
     k.u[0] = k_update_yz<0, LOYZ>; k.u[1] = k_update_yz<1, LOYZ>; k.u[2] = k_update_yz<2, LOYZ>; k.u[3] = k_update_yz<3, LOYZ>;
-    k.d_x = k_dens_x<LOXZ>;
-    k.name = name;
+    k.d_x = k_dens_x<LOXZ>; k.d_yz = nullptr;
+    k.name = name; k.v5 = 0;
     return k;
 }
-// ---- v4 plane kernels: compile-time choice of unit size (NCOMP), prefetch depth (NBUF), warps, staging ----
+// ---- plane5 kernels: compile-time choice of unit size (NCOMP), prefetch depth (NBUF), warps, staging ----
 static constexpr size_t SMEM_LIMIT = 227 * 1024;
-static constexpr size_t v4_smem_happly_yz(int ny, int nz, int ncomp, int nbuf, bool vstage)
+template <int N> static constexpr size_t tabsz() { return (size_t)LOp<N>::TABSZ; }
+template <int NY, int NZ>
+static constexpr size_t v5_smem_happly_yz(int ncomp, int nbuf, bool vstage)
 {
-    return 16 * (size_t)(2 * ny + 2 * nz) + 16 * (size_t)(ny * ldpad(nz)) * ncomp * (nbuf + 1)
-         + 8 * (size_t)(ny * ldpad(nz)) * (6 + (vstage ? 6 : 0));
+    return 8 * ((tabsz<NY>() + tabsz<NZ>() + 1) / 2 * 2) + 16 * (size_t)(NY * ldpad(NZ)) * ncomp * (nbuf + 1)
+         + 8 * (size_t)(NY * ldpad(NZ)) * (6 + (vstage ? 6 : 0));
 }
-static constexpr size_t v4_smem_happly_xz(int nx, int nz, int ncomp, int nbuf)
+template <int NX, int NZ>
+static constexpr size_t v5_smem_happly_xz(int ncomp, int nbuf, int nwarp)
 {
-    return 16 * (size_t)(2 * nx) + 16 * (size_t)(nx * ldpad(nz)) * ncomp * 2 * nbuf + 8 * (size_t)(nx * ldpad(nz)) * 4 + 8 * 64;
+    return 8 * ((tabsz<NX>() + 1) / 2 * 2) + 16 * (size_t)(NX * ldpad(NZ)) * ncomp * nbuf + 8 * (size_t)(NX * ldpad(NZ)) * 4 + 8 * 2 * nwarp;
 }
-static constexpr size_t v4_smem_update(int ny, int nz) { return 16 * (size_t)(2 * ny + 2 * nz) + 16 * (size_t)(2 * ny * ldpad(nz)); }
-static constexpr size_t v4_smem_dens_x(int nx, int nz) { return 16 * (size_t)(2 * nx) + 16 * (size_t)(2 * nx * ldpad(nz)); }
+template <int NY, int NZ>
+static constexpr size_t v5_smem_dens_yz() { return 8 * ((tabsz<NY>() + tabsz<NZ>() + 1) / 2 * 2) + 16 * (size_t)(4 * NY * ldpad(NZ)); }
+template <int NX, int NZ>
+static constexpr size_t v5_smem_dens_x() { return 8 * ((tabsz<NX>() + 1) / 2 * 2) + 16 * (size_t)(4 * NX * ldpad(NZ)); }
 static constexpr int imin(int a, int b) { return a < b ? a : b; }
 static constexpr int imax(int a, int b) { return a > b ? a : b; }
-// warps of an H-apply CTA: one strip task per warp if possible; long lines need more registers per thread
-static constexpr int v4_warps_h(int tasks, int nline) { return imin(tasks, nline >= 32 ? 8 : 12); }
+// warps per 2-spinor of an H-apply CTA: one strip task per warp if possible; long lines need more registers per thread
+static constexpr int v5_wpp(int npair, int strips, int nline) { return imin(strips, (nline >= 40 ? 8 : 12) / npair); }
 
 template <int NX, int NY, int NZ>
-static KernSet make_v4_set()
+static KernSet make_v5_set()
 {
     // yz: prefer whole states with prefetch, then 2-spinors with prefetch, then 2-spinors without
-    constexpr int CYZ = (v4_smem_happly_yz(NY, NZ, 4, 2, false) <= SMEM_LIMIT) ? 4 : 2;
-    constexpr int BYZ = (v4_smem_happly_yz(NY, NZ, CYZ, 2, false) <= SMEM_LIMIT) ? 2 : 1;
-    constexpr bool VST = v4_smem_happly_yz(NY, NZ, CYZ, BYZ, true) <= SMEM_LIMIT;
-    constexpr int WYZ = v4_warps_h((CYZ / 2) * imax(NY, NZ) / 4, imax(NY, NZ));
-    constexpr int CXZ = (v4_smem_happly_xz(NX, NZ, 4, 2) <= SMEM_LIMIT) ? 4 : 2;
-    constexpr int BXZ = (v4_smem_happly_xz(NX, NZ, CXZ, 2) <= SMEM_LIMIT) ? 2 : 1;
-    constexpr int WXZ = v4_warps_h((CXZ / 2) * NZ / 4, NX);
-    constexpr int WU = imin(2 * imax(NY, NZ) / 4, imax(NY, NZ) >= 32 ? 8 : 12);
-    constexpr int WD = imin(2 * NZ / 4, imax(NX, NZ) >= 32 ? 8 : 12);
-    static_assert(v4_smem_happly_yz(NY, NZ, CYZ, BYZ, VST) <= SMEM_LIMIT, "yz plane too large");
-    static_assert(v4_smem_happly_xz(NX, NZ, CXZ, BXZ) <= SMEM_LIMIT, "xz plane too large");
+    constexpr int CYZ = (v5_smem_happly_yz<NY, NZ>(4, 2, false) <= SMEM_LIMIT) ? 4 : 2;
+    constexpr int BYZ = (v5_smem_happly_yz<NY, NZ>(CYZ, 2, false) <= SMEM_LIMIT) ? 2 : 1;
+    constexpr bool VST = v5_smem_happly_yz<NY, NZ>(CYZ, BYZ, true) <= SMEM_LIMIT;
+    constexpr int WYZ = (CYZ / 2) * v5_wpp(CYZ / 2, imax(NY, NZ) / 4, imax(NY, NZ));
+    constexpr int WXZ0 = 12;
+    constexpr int CXZ = (v5_smem_happly_xz<NX, NZ>(4, 2, WXZ0) <= SMEM_LIMIT) ? 4 : 2;
+    constexpr int BXZ = (v5_smem_happly_xz<NX, NZ>(CXZ, 2, WXZ0) <= SMEM_LIMIT) ? 2 : 1;
+    constexpr int WXZ = imin((CXZ / 2) * NZ / 4, NX >= 40 ? 8 : 12);
+    constexpr int WDY = imin(2 * (NY / 4) + 2 * (NZ / 4), imax(NY, NZ) >= 40 ? 8 : 12);
+    constexpr int WDX = imin(2 * NZ / 4, NX >= 40 ? 8 : 12);
+    static_assert(v5_smem_happly_yz<NY, NZ>(CYZ, BYZ, VST) <= SMEM_LIMIT, "yz plane too large");
+    static_assert(v5_smem_happly_xz<NX, NZ>(CXZ, BXZ, WXZ) <= SMEM_LIMIT, "xz plane too large");
     KernSet k;
-    k.h_yz = k4_happly_yz<NY, NZ, CYZ, BYZ, WYZ, VST>; k.h_xz = k4_happly_xz<NX, NZ, CXZ, BXZ, WXZ>;
-    k.u[0] = k4_update_yz<0, NY, NZ, WU>; k.u[1] = k4_update_yz<1, NY, NZ, WU>;
-    k.u[2] = k4_update_yz<2, NY, NZ, WU>; k.u[3] = k4_update_yz<3, NY, NZ, WU>;
-    k.d_x = k4_dens_x<NX, NZ, WD>;
-    k.name = "dmma";
-    k.thr_h[0] = 32 * WYZ; k.thr_h[1] = 32 * WXZ; k.thr_u = 32 * WU; k.thr_d = 32 * WD;
-    k.smem_h[0] = v4_smem_happly_yz(NY, NZ, CYZ, BYZ, VST); k.smem_h[1] = v4_smem_happly_xz(NX, NZ, CXZ, BXZ);
-    k.smem_u = v4_smem_update(NY, NZ); k.smem_d = v4_smem_dens_x(NX, NZ);
+    k.h_yz = k5_happly_yz<NY, NZ, CYZ, BYZ, WYZ, VST>; k.h_xz = k5_happly_xz<NX, NZ, CXZ, BXZ, WXZ>;
+    k.u[0] = nullptr; k.u[1] = k5_update<1>; k.u[2] = k5_update<2>; k.u[3] = k5_update<3>;
+    k.d_yz = k5_dens_yz<NY, NZ, WDY>; k.d_x = k5_dens_x<NX, NZ, WDX>;
+    k.name = "dmma"; k.v5 = 1;
+    k.thr_h[0] = 32 * WYZ; k.thr_h[1] = 32 * WXZ; k.thr_u = LISE_UPD_THREADS; k.thr_d = 32 * WDX; k.thr_dyz = 32 * WDY;
+    k.smem_h[0] = v5_smem_happly_yz<NY, NZ>(CYZ, BYZ, VST); k.smem_h[1] = v5_smem_happly_xz<NX, NZ>(CXZ, BXZ, WXZ);
+    k.smem_u = 0; k.smem_d = v5_smem_dens_x<NX, NZ>(); k.smem_dyz = v5_smem_dens_yz<NY, NZ>();
     k.ups_xz = 4 / CXZ;
     return k;
 }
@@ -226,16 +298,16 @@ static KernSet make_v4_set()
 static bool pick_kernels(int nx, int ny, int nz, int R, bool want_mma, KernSet* out)
 {
     if (want_mma) {
-#define X(a, b, c_) if (nx == a && ny == b && nz == c_) { *out = make_v4_set<a, b, c_>(); return true; }
+#define X(a, b, c_) if (nx == a && ny == b && nz == c_) { *out = make_v5_set<a, b, c_>(); return true; }
         LISE_MMA_SHAPES(X)
 #undef X
     }
     if (R == 8) *out = make_set<DenseLines<8>, DenseLines<8>>("dense");
     else if (R == 4) *out = make_set<DenseLines<4>, DenseLines<4>>("dense");
     else *out = make_set<DenseLines<2>, DenseLines<2>>("dense");
-    out->thr_h[0] = out->thr_h[1] = out->thr_u = out->thr_d = 0;
-    out->smem_h[0] = out->smem_h[1] = out->smem_u = out->smem_d = 0;
-    out->ups_xz = 1;
+    out->thr_h[0] = out->thr_h[1] = out->thr_u = out->thr_d = out->thr_dyz = 0;
+    out->smem_h[0] = out->smem_h[1] = out->smem_u = out->smem_d = out->smem_dyz = 0;
+    out->ups_xz = 1; out->v5 = 0; out->d_yz = nullptr;
     return false;
 }
 
@@ -249,13 +321,20 @@ static int launch_happly(lise_ctx* c, const HArgs& a)
     CKL();
     return LISE_OK;
 }
+// MODE 1, 2: ABM (Eq. 78); 3: starter Taylor term; 0: densities of u.Z only (generic kernels).  `st`: launch stream
 template <int MODE>
-static int launch_update(lise_ctx* c, const UArgs& a)
+static int launch_update(lise_ctx* c, const UArgs& a, cudaStream_t st)
 {
-    dim3 grid(c->L.nx, c->G);
-    prof_begin(c, PC_UPDATE);
-    c->ks.u[MODE]<<<grid, c->ks.thr_u, c->ks.smem_u, c->stream>>>(a);
-    prof_end(c);
+    prof_begin(c, PC_UPDATE, st);
+    if (c->ks.v5) {
+        const size_t slen = (size_t)4 * c->L.nxyz, per = (size_t)LISE_UPD_THREADS * LISE_UPD_EPT;
+        dim3 grid((unsigned)((slen + per - 1) / per), a.ns);
+        c->ks.u[MODE]<<<grid, LISE_UPD_THREADS, 0, st>>>(a);
+    } else {
+        dim3 grid(c->L.nx, c->G);
+        c->ks.u[MODE]<<<grid, c->ks.thr_u, c->ks.smem_u, st>>>(a);
+    }
+    prof_end(c, st);
     CKL();
     return LISE_OK;
 }
@@ -268,39 +347,60 @@ static int launch_dens_x(lise_ctx* c, const DArgs& a)
     CKL();
     return LISE_OK;
 }
+static int launch_dens_yz(lise_ctx* c, const DArgs& a)
+{
+    dim3 grid(c->L.nx, c->G);
+    prof_begin(c, PC_DENS_YZ);
+    c->ks.d_yz<<<grid, c->ks.thr_dyz, c->ks.smem_dyz, c->stream>>>(a);
+    prof_end(c);
+    CKL();
+    return LISE_OK;
+}
 static int set_attrs(lise_ctx* c)
 {
     CK(cudaFuncSetAttribute(c->ks.h_yz, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->ks.smem_h[0]));
     CK(cudaFuncSetAttribute(c->ks.h_xz, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->ks.smem_h[1]));
-    for (int m = 0; m < 4; ++m) CK(cudaFuncSetAttribute(c->ks.u[m], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->ks.smem_u));
+    if (!c->ks.v5)
+        for (int m = 0; m < 4; ++m) CK(cudaFuncSetAttribute(c->ks.u[m], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->ks.smem_u));
     CK(cudaFuncSetAttribute(c->ks.d_x, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->ks.smem_d));
+    if (c->ks.d_yz) CK(cudaFuncSetAttribute(c->ks.d_yz, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->ks.smem_dyz));
     return LISE_OK;
 }
 
 static void fill_common(lise_ctx* c, const double2** ct) { for (int i = 0; i < 3; ++i) ct[i] = c->ctab[i]; }
+static void fill_stab(lise_ctx* c, const double** st) { for (int i = 0; i < 3; ++i) st[i] = c->stab[i]; }
+static inline int neta(const lise_ctx* c) { return c->ks.ups_xz * c->L.ny; }
+static inline cplx* Wbuf(lise_ctx* c, int b) { return c->W + (size_t)b * c->wcap * 4 * c->L.nxyz; }
+static inline double* etabuf(lise_ctx* c, int b) { return c->eta_part + (size_t)b * c->wcap * neta(c); }
 
-// W = H X for ns states (ns <= chunk) of species q
-static int apply_h_chunk(lise_ctx* c, int q, const cplx* X, cplx* W, int ns)
+// W = H X for ns states (ns <= chunk) of species q; eta partial sums -> eta (buffer of ns * neta doubles)
+static int apply_h_chunk(lise_ctx* c, int q, const cplx* X, cplx* W, double* eta, int ns)
 {
     HArgs a;
-    a.L = c->L; a.X = X; a.W = W; a.pot = c->pot[q]; fill_common(c, a.ctab);
-    a.eta_part = c->eta_part; a.ns = ns; a.G = c->G;
+    a.L = c->L; a.X = X; a.W = W; a.pot = c->pot[q]; fill_common(c, a.ctab); fill_stab(c, a.stab);
+    a.eta_part = eta; a.ns = ns; a.G = c->G;
     TRY(launch_happly<0>(c, a));
     TRY(launch_happly<1>(c, a));
     return LISE_OK;
 }
 
-static UArgs make_uargs(lise_ctx* c, int q, size_t off, int ns)
+static UArgs make_uargs(lise_ctx* c, int q, size_t off, int ns, int wb)
 {
     UArgs u;
-    u.L = c->L; u.W = c->W;
+    u.L = c->L; u.W = Wbuf(c, wb);
     u.sA = S(c, q, RA) + off; u.sB = S(c, q, RB) + off; u.sC = S(c, q, RC) + off; u.sD = S(c, q, RD) + off;
     u.sE = S(c, q, RE) + off; u.sF = S(c, q, RF) + off; u.sG = S(c, q, RG) + off;
-    u.Z = nullptr; u.eta_part = c->eta_part; u.eta_fix = c->eta_fix; u.part = c->part[q];
+    u.Z = nullptr; u.eta_part = etabuf(c, wb); u.eta_fix = c->eta_fix; u.part = c->part[q];
     fill_common(c, u.ctab);
-    u.neta = c->ks.ups_xz * c->L.ny; u.dt = c->dt; u.hbarc = c->par.hbarc; u.ns = ns; u.G = c->G; u.order = 0; u.remove_phase = c->par.remove_phase;
+    u.neta = neta(c); u.dt = c->dt; u.hbarc = c->par.hbarc; u.ns = ns; u.G = c->G; u.order = 0; u.remove_phase = c->par.remove_phase;
     u.write_f = 1;
     return u;
+}
+static DArgs make_dargs(lise_ctx* c, int q, const cplx* Z, int ns)
+{
+    DArgs d;
+    d.L = c->L; d.Z = Z; d.part = c->part[q]; fill_common(c, d.ctab); fill_stab(c, d.stab); d.ns = ns; d.G = c->G;
+    return d;
 }
 
 static int zero_partials(lise_ctx* c, int q)
@@ -309,17 +409,24 @@ static int zero_partials(lise_ctx* c, int q)
     return LISE_OK;
 }
 
-// part[q] += densities of the nwf[q] states in Z (both passes)
+// part[q] += densities of the ns states in Z (all passes), on the context's stream
+static int dens_chunk(lise_ctx* c, int q, const cplx* Z, int ns)
+{
+    if (c->ks.v5) TRY(launch_dens_yz(c, make_dargs(c, q, Z, ns)));
+    else {
+        UArgs u = make_uargs(c, q, 0, ns, 0);
+        u.Z = Z;
+        TRY(launch_update<0>(c, u, c->stream));
+    }
+    TRY(launch_dens_x(c, make_dargs(c, q, Z, ns)));
+    return LISE_OK;
+}
 static int dens_accumulate(lise_ctx* c, int q, const cplx* Z)
 {
     const size_t slen = (size_t)4 * c->L.nxyz;
     for (int s0 = 0; s0 < c->nwf[q]; s0 += c->chunk) {
         const int ns = (c->nwf[q] - s0 < c->chunk) ? c->nwf[q] - s0 : c->chunk;
-        UArgs u = make_uargs(c, q, 0, ns);
-        u.Z = Z + s0 * slen;
-        TRY(launch_update<0>(c, u));
-        DArgs d; d.L = c->L; d.Z = Z + s0 * slen; d.part = c->part[q]; fill_common(c, d.ctab); d.ns = ns; d.G = c->G;
-        TRY(launch_dens_x(c, d));
+        TRY(dens_chunk(c, q, Z + s0 * slen, ns));
     }
     return LISE_OK;
 }
@@ -397,25 +504,47 @@ static void rotate_f(lise_ctx* c)
     c->role[RD] = rc; c->role[RE] = rd; c->role[RC] = re;
 }
 
-// one ABM predictor-modifier-corrector step (Eq. 78)
+// one ABM predictor-modifier-corrector step (Eq. 78).
+// plane5 kernels: software pipeline over chunks -- the DMMA-bound kernels (H-apply of chunk i + 1, densities of
+// chunk i - 1) run on the context's stream while the HBM-bound update of chunk i runs on stream2; W and the eta
+// partial sums are double-buffered.  Everything is joined back into the context's stream before returning.
 static int abm_step(lise_ctx* c)
 {
     const size_t slen = (size_t)4 * c->L.nxyz;
     TRY(ensure_potentials(c));                      // potentials of y_n
+    const bool pipe = c->ks.v5 && c->overlap;
     for (int phase = 1; phase <= 2; ++phase) {
         TRY(zero_partials(c, 0)); TRY(zero_partials(c, 1));
+        int i = 0;                                  // chunk counter across both species
+        int pq = -1, pns = 0; size_t poff = 0;      // previous chunk: its densities are still to be accumulated
         for (int q = 0; q < 2; ++q)
-            for (int s0 = 0; s0 < c->nwf[q]; s0 += c->chunk) {
+            for (int s0 = 0; s0 < c->nwf[q]; s0 += c->chunk, ++i) {
                 const int ns = (c->nwf[q] - s0 < c->chunk) ? c->nwf[q] - s0 : c->chunk;
                 const size_t off = s0 * slen;
+                const int wb = pipe ? (i & 1) : 0;
                 const cplx* X = (phase == 1 ? S(c, q, RA) : S(c, q, RF)) + off;
-                TRY(apply_h_chunk(c, q, X, c->W, ns));
-                UArgs u = make_uargs(c, q, off, ns);
-                if (phase == 1) TRY(launch_update<1>(c, u)); else TRY(launch_update<2>(c, u));
-                DArgs d; d.L = c->L; d.Z = (phase == 1 ? S(c, q, RF) : S(c, q, RB)) + off; d.part = c->part[q];
-                fill_common(c, d.ctab); d.ns = ns; d.G = c->G;
-                TRY(launch_dens_x(c, d));
+                TRY(apply_h_chunk(c, q, X, Wbuf(c, wb), etabuf(c, wb), ns));
+                UArgs u = make_uargs(c, q, off, ns, wb);
+                cudaStream_t su = pipe ? c->stream2 : c->stream;
+                if (pipe) { CK(cudaEventRecord(c->ev_h[wb], c->stream)); CK(cudaStreamWaitEvent(c->stream2, c->ev_h[wb], 0)); }
+                if (phase == 1) TRY(launch_update<1>(c, u, su)); else TRY(launch_update<2>(c, u, su));
+                if (pipe) CK(cudaEventRecord(c->ev_u[wb], c->stream2));
+                if (c->ks.v5) {
+                    if (pipe) {
+                        if (pq >= 0) {              // densities of the previous chunk, behind this chunk's H-apply
+                            CK(cudaStreamWaitEvent(c->stream, c->ev_u[wb ^ 1], 0));
+                            TRY(dens_chunk(c, pq, (phase == 1 ? S(c, pq, RF) : S(c, pq, RB)) + poff, pns));
+                        }
+                        pq = q; pns = ns; poff = off;
+                    } else TRY(dens_chunk(c, q, (phase == 1 ? S(c, q, RF) : S(c, q, RB)) + off, ns));
+                } else {
+                    TRY(launch_dens_x(c, make_dargs(c, q, (phase == 1 ? S(c, q, RF) : S(c, q, RB)) + off, ns)));
+                }
             }
+        if (pipe && pq >= 0) {
+            CK(cudaStreamWaitEvent(c->stream, c->ev_u[(i - 1) & 1], 0));
+            TRY(dens_chunk(c, pq, (phase == 1 ? S(c, pq, RF) : S(c, pq, RB)) + poff, pns));
+        }
         if (phase == 1) TRY(grid_phase(c, 1));     // potentials of the modifier m
     }
     // y_{n+1} sits in B: A <-> B; f history shifts
@@ -435,10 +564,10 @@ static int taylor4_all(lise_ctx* c, int write_f)
             const size_t off = s0 * slen;
             for (int m = 1; m <= 4; ++m) {
                 const cplx* X = (m == 1 ? S(c, q, RA) : S(c, q, RG)) + off;
-                TRY(apply_h_chunk(c, q, X, c->W, ns));
-                UArgs u = make_uargs(c, q, off, ns);
+                TRY(apply_h_chunk(c, q, X, Wbuf(c, 0), etabuf(c, 0), ns));
+                UArgs u = make_uargs(c, q, off, ns, 0);
                 u.order = m; u.write_f = write_f;
-                TRY(launch_update<3>(c, u));
+                TRY(launch_update<3>(c, u, c->stream));
             }
         }
     return LISE_OK;
@@ -589,6 +718,20 @@ static int ctx_init(lise_ctx* c)
         DM(c->ctab[i], t.size());
         CK(cudaMemcpy(c->ctab[i], t.data(), sizeof(double2) * t.size(), cudaMemcpyHostToDevice));
     }
+    for (int i = 0; i < 3; ++i) {
+        std::vector<double> t;
+        host_stab(c->n[i], L.dx, t);
+        DM(c->stab[i], t.size());
+        CK(cudaMemcpy(c->stab[i], t.data(), sizeof(double) * t.size(), cudaMemcpyHostToDevice));
+    }
+    TRY(upload_rdft());
+    CK(cudaStreamCreateWithFlags(&c->stream2, cudaStreamNonBlocking));
+    for (int i = 0; i < 2; ++i) {
+        CK(cudaEventCreateWithFlags(&c->ev_h[i], cudaEventDisableTiming));
+        CK(cudaEventCreateWithFlags(&c->ev_u[i], cudaEventDisableTiming));
+    }
+    c->overlap = 1;
+    if (const char* e = getenv("LISE_OVERLAP")) c->overlap = atoi(e) ? 1 : 0;
     // state slots and scratch
     for (int q = 0; q < 2; ++q)
         for (int s = 0; s < LISE_NSLOT; ++s) {
@@ -596,10 +739,10 @@ static int ctx_init(lise_ctx* c)
             CK(cudaMemset(c->slot[q][s], 0, sizeof(cplx) * (size_t)c->nwf[q] * 4 * nx));
         }
     for (int s = 0; s < LISE_NSLOT; ++s) c->role[s] = s;
-    c->wcap = nmax < 512 ? (nmax > 0 ? nmax : 1) : 512;     // largest chunk lise_set_chunk accepts
+    c->wcap = nmax < 256 ? (nmax > 0 ? nmax : 1) : 256;     // largest chunk lise_set_chunk accepts
     if (c->wcap < c->chunk) c->wcap = c->chunk;
-    DM(c->W, (size_t)c->wcap * 4 * nx);
-    DM(c->eta_part, (size_t)c->wcap * L.ny * 2);
+    DM(c->W, (size_t)2 * c->wcap * 4 * nx);
+    DM(c->eta_part, (size_t)2 * c->wcap * L.ny * 2);
     DM(c->eta_fix, (size_t)c->wcap);
     for (int q = 0; q < 2; ++q) {
         DM(c->part[q], (size_t)LISE_MAXG * LISE_NACC * nx);
@@ -666,6 +809,8 @@ extern "C" void lise_destroy(lise_ctx* c)
 {
     if (!c) return;
     cudaStreamSynchronize(c->stream);
+    if (c->stream2) { cudaStreamSynchronize(c->stream2); cudaStreamDestroy(c->stream2); }
+    for (int i = 0; i < 2; ++i) { if (c->ev_h[i]) cudaEventDestroy(c->ev_h[i]); if (c->ev_u[i]) cudaEventDestroy(c->ev_u[i]); }
     if (c->allocs) {
         for (void* p : *c->allocs) cudaFree(p);
         delete c->allocs;
@@ -703,6 +848,13 @@ extern "C" int lise_set_chunk(lise_ctx* c, int n)
     if (!c) return LISE_EINVAL;
     if (n <= 0) c->chunk = default_chunk(c);
     else c->chunk = n > c->wcap ? c->wcap : n;
+    return LISE_OK;
+}
+
+extern "C" int lise_set_overlap(lise_ctx* c, int enable)
+{
+    if (!c) return LISE_EINVAL;
+    c->overlap = enable ? 1 : 0;
     return LISE_OK;
 }
 
@@ -790,7 +942,7 @@ extern "C" int lise_apply_h(lise_ctx* c, int q, const void* in_dev, void* out_de
     const int ch = c->chunk;                       // eta_part scratch is sized for wcap >= chunk states
     for (int s0 = 0; s0 < nstates; s0 += ch) {
         const int ns = (nstates - s0 < ch) ? nstates - s0 : ch;
-        TRY(apply_h_chunk(c, q, (const cplx*)in_dev + s0 * slen, (cplx*)out_dev + s0 * slen, ns));
+        TRY(apply_h_chunk(c, q, (const cplx*)in_dev + s0 * slen, (cplx*)out_dev + s0 * slen, etabuf(c, 0), ns));
     }
     return LISE_OK;
 }

@@ -270,7 +270,8 @@ struct HArgs {
     const cplx* X;
     cplx* W;
     const double* pot;        // [LISE_NPOT][nxyz]
-    const double2* ctab[3];   // doubled circulant tables per axis (global)
+    const double2* ctab[3];   // doubled circulant tables per axis (global; generic kernels)
+    const double* stab[3];    // block-diagonalised tables per axis (split_lineop.cuh; plane5 kernels)
     double* eta_part;         // [ns][ny]
     int ns, G;
 };
@@ -563,6 +564,7 @@ struct DArgs {
     const cplx* Z;
     double* part;
     const double2* ctab[3];
+    const double* stab[3];
     int ns, G;
 };
 template <class LO>

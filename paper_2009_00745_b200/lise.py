@@ -29,7 +29,7 @@ class Observables(C.Structure):
 
 
 EXPORTS = ["lise_default_params", "lise_create", "lise_destroy", "lise_set_params", "lise_set_stream",
-           "lise_set_dt", "lise_set_chunk", "lise_set_wavefunctions", "lise_get_wavefunctions",
+           "lise_set_dt", "lise_set_chunk", "lise_set_overlap", "lise_set_wavefunctions", "lise_get_wavefunctions",
            "lise_upload_wavefunctions", "lise_download_wavefunctions", "lise_set_reduce_hook",
            "lise_densities", "lise_potentials", "lise_apply_h", "lise_step", "lise_observables",
            "lise_profile", "lise_profile_read", "lise_measure_fp64_peak", "lise_line_operator", "lise_launch_count", "lise_device_bytes", "lise_strerror", "lise_last_error"]
@@ -69,6 +69,7 @@ def load():
     lib.lise_set_stream.argtypes = [vp, vp]
     lib.lise_set_dt.argtypes = [vp, dp]
     lib.lise_set_chunk.argtypes = [vp, ip]
+    lib.lise_set_overlap.argtypes = [vp, ip]
     lib.lise_set_wavefunctions.argtypes = [vp, ip, vp]
     lib.lise_get_wavefunctions.argtypes = [vp, ip, vp]
     lib.lise_upload_wavefunctions.argtypes = [vp, ip, vp, ip]
@@ -171,6 +172,9 @@ class Lise:
     def set_chunk(self, n):
         self._chk(self.lib.lise_set_chunk(self._h, n), "lise_set_chunk")
 
+    def set_overlap(self, enable):
+        self._chk(self.lib.lise_set_overlap(self._h, int(enable)), "lise_set_overlap")
+
     def set_wavefunctions(self, q, psi):
         p = self._dev(psi, torch.complex128, self.nwf[q] * 4 * self.nxyz) if self.nwf[q] else C.c_void_p()
         self._chk(self.lib.lise_set_wavefunctions(self._h, q, p), "lise_set_wavefunctions")
@@ -243,13 +247,13 @@ class Lise:
         self._chk(self.lib.lise_observables(self._h, C.byref(o)), "lise_observables")
         return o.as_dict()
 
-    PROFILE_CLASSES = ("happly_yz", "happly_xz", "update_yz", "dens_x", "grid")
+    PROFILE_CLASSES = ("happly_yz", "happly_xz", "update", "dens_x", "grid", "dens_yz")
 
     def profile(self, enable=True):
         self._chk(self.lib.lise_profile(self._h, int(enable)), "lise_profile")
 
     def profile_read(self):
-        ms = (C.c_double * 5)(); cnt = (C.c_long * 5)()
+        ms = (C.c_double * 6)(); cnt = (C.c_long * 6)()
         self._chk(self.lib.lise_profile_read(self._h, ms, cnt), "lise_profile_read")
         return {n: (ms[i], cnt[i]) for i, n in enumerate(self.PROFILE_CLASSES)}
 
