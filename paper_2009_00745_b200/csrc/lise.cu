@@ -28,6 +28,7 @@ struct KernSet {
     int thr_h[2], thr_u, thr_d, thr_dyz;   // threads per CTA: happly yz / xz, update, dens_x, dens_yz
     size_t smem_h[2], smem_u, smem_d, smem_dyz;   // dynamic shared memory, bytes (0 = filled by ctx_init for the generic path)
     int ups_xz;                            // eta partial sums per state = ups_xz * ny
+    int cps_h[2];                          // resident CTAs per SM of the two H-apply kernels (state groups = G * cps)
 };
 struct lise_ctx {
     Lattice L;
@@ -41,7 +42,7 @@ struct lise_ctx {
     double* stab[3];                        // block-diagonalised line-operator tables (split_lineop.cuh)
     cudaStream_t stream2;                   // the HBM-bound update kernels run here, overlapping the DMMA kernels
     cudaEvent_t ev_h[2], ev_u[2];
-    int overlap;
+    int overlap, dgroup;                    // dgroup: chunks per density-kernel launch
     cplx* slot[2][LISE_NSLOT];
     int role[LISE_NSLOT];
     cplx* W;                                // [2][wcap] states: H-apply output, double-buffered across chunks
@@ -262,24 +263,47 @@ static constexpr int imax(int a, int b) { return a > b ? a : b; }
 // warps per 2-spinor of an H-apply CTA: one strip task per warp if possible; long lines need more registers per thread
 static constexpr int v5_wpp(int npair, int strips, int nline) { return imin(strips, (nline >= 40 ? 8 : 12) / npair); }
 
-template <int NX, int NY, int NZ>
+// register cap of an H-apply kernel with `warps` warps and `ctas` CTAs per SM; 4 warps x 128 registers stay free for
+// the co-resident update CTA
+static constexpr int v5_maxr(int warps, int ctas)
+{
+    const int r = ((65536 - 4 * 32 * 128) / (warps * 32 * ctas)) & ~7;
+    return r > 255 ? 255 : r;
+}
+// warps for `tasks` equal tasks per pass: all of them if they fit under `cap`, else the largest count <= cap that
+// divides them evenly
+static constexpr int v5_warps(int tasks, int cap)
+{
+    if (tasks <= cap) return tasks;
+    for (int w = cap; w >= cap / 2; --w) if (tasks % w == 0) return w;
+    return cap;
+}
+// VAR 0: one plane-owner CTA per SM, whole states if shared memory allows.
+// VAR 1: two CTAs per SM working on 2-spinors (their barrier and epilogue phases interleave) where two fit.
+static constexpr size_t SMEM_HALF = (228 * 1024) / 2 - 1024;
+template <int NX, int NY, int NZ, int VAR>
 static KernSet make_v5_set()
 {
+    constexpr bool TWO_YZ = VAR == 1 && v5_smem_happly_yz<NY, NZ>(2, 2, false) <= SMEM_HALF && imax(NY, NZ) / 4 <= 8;
+    constexpr bool TWO_XZ = VAR == 1 && v5_smem_happly_xz<NX, NZ>(2, 2, 8) <= SMEM_HALF && NZ / 4 <= 8;
     // yz: prefer whole states with prefetch, then 2-spinors with prefetch, then 2-spinors without
-    constexpr int CYZ = (v5_smem_happly_yz<NY, NZ>(4, 2, false) <= SMEM_LIMIT) ? 4 : 2;
+    constexpr int CYZ = TWO_YZ ? 2 : (v5_smem_happly_yz<NY, NZ>(4, 2, false) <= SMEM_LIMIT) ? 4 : 2;
     constexpr int BYZ = (v5_smem_happly_yz<NY, NZ>(CYZ, 2, false) <= SMEM_LIMIT) ? 2 : 1;
-    constexpr bool VST = v5_smem_happly_yz<NY, NZ>(CYZ, BYZ, true) <= SMEM_LIMIT;
-    constexpr int WYZ = (CYZ / 2) * v5_wpp(CYZ / 2, imax(NY, NZ) / 4, imax(NY, NZ));
+    constexpr bool VST = !TWO_YZ && v5_smem_happly_yz<NY, NZ>(CYZ, BYZ, true) <= SMEM_LIMIT;
+    constexpr int WYZ = TWO_YZ ? imax(NY, NZ) / 4 : (CYZ / 2) * v5_wpp(CYZ / 2, imax(NY, NZ) / 4, imax(NY, NZ));
     constexpr int WXZ0 = 12;
-    constexpr int CXZ = (v5_smem_happly_xz<NX, NZ>(4, 2, WXZ0) <= SMEM_LIMIT) ? 4 : 2;
+    constexpr int CXZ = TWO_XZ ? 2 : (v5_smem_happly_xz<NX, NZ>(4, 2, WXZ0) <= SMEM_LIMIT) ? 4 : 2;
     constexpr int BXZ = (v5_smem_happly_xz<NX, NZ>(CXZ, 2, WXZ0) <= SMEM_LIMIT) ? 2 : 1;
-    constexpr int WXZ = imin((CXZ / 2) * NZ / 4, NX >= 40 ? 8 : 12);
+    constexpr int WXZ = TWO_XZ ? NZ / 4 : v5_warps((CXZ / 2) * NZ / 4, NX >= 32 ? 8 : 12);
     constexpr int WDY = imin(2 * (NY / 4) + 2 * (NZ / 4), imax(NY, NZ) >= 40 ? 8 : 12);
     constexpr int WDX = imin(2 * NZ / 4, NX >= 40 ? 8 : 12);
     static_assert(v5_smem_happly_yz<NY, NZ>(CYZ, BYZ, VST) <= SMEM_LIMIT, "yz plane too large");
     static_assert(v5_smem_happly_xz<NX, NZ>(CXZ, BXZ, WXZ) <= SMEM_LIMIT, "xz plane too large");
     KernSet k;
-    k.h_yz = k5_happly_yz<NY, NZ, CYZ, BYZ, WYZ, VST>; k.h_xz = k5_happly_xz<NX, NZ, CXZ, BXZ, WXZ>;
+    // register caps: 128 where a 12-warp CTA then leaves room for one update CTA per SM (overlap), else what fits
+    constexpr int RYZ = TWO_YZ ? v5_maxr(WYZ, 2) : v5_maxr(WYZ, 1), RXZ = TWO_XZ ? v5_maxr(WXZ, 2) : v5_maxr(WXZ, 1);
+    k.h_yz = k5_happly_yz<NY, NZ, CYZ, BYZ, WYZ, VST, RYZ>; k.h_xz = k5_happly_xz<NX, NZ, CXZ, BXZ, WXZ, RXZ>;
+    k.cps_h[0] = TWO_YZ ? 2 : 1; k.cps_h[1] = TWO_XZ ? 2 : 1;
     k.u[0] = nullptr; k.u[1] = k5_update<1>; k.u[2] = k5_update<2>; k.u[3] = k5_update<3>;
     k.d_yz = k5_dens_yz<NY, NZ, WDY>; k.d_x = k5_dens_x<NX, NZ, WDX>;
     k.name = "dmma"; k.v5 = 1;
@@ -298,7 +322,10 @@ static KernSet make_v5_set()
 static bool pick_kernels(int nx, int ny, int nz, int R, bool want_mma, KernSet* out)
 {
     if (want_mma) {
-#define X(a, b, c_) if (nx == a && ny == b && nz == c_) { *out = make_v5_set<a, b, c_>(); return true; }
+        int var = 0;
+        if (const char* e = getenv("LISE_HVAR")) var = atoi(e);
+        if (var == 1 && nx == 24 && ny == 24 && nz == 24) { *out = make_v5_set<24, 24, 24, 1>(); return true; }
+#define X(a, b, c_) if (nx == a && ny == b && nz == c_) { *out = make_v5_set<a, b, c_, 0>(); return true; }
         LISE_MMA_SHAPES(X)
 #undef X
     }
@@ -307,16 +334,18 @@ static bool pick_kernels(int nx, int ny, int nz, int R, bool want_mma, KernSet* 
     else *out = make_set<DenseLines<2>, DenseLines<2>>("dense");
     out->thr_h[0] = out->thr_h[1] = out->thr_u = out->thr_d = out->thr_dyz = 0;
     out->smem_h[0] = out->smem_h[1] = out->smem_u = out->smem_d = out->smem_dyz = 0;
-    out->ups_xz = 1; out->v5 = 0; out->d_yz = nullptr;
+    out->ups_xz = 1; out->v5 = 0; out->d_yz = nullptr; out->cps_h[0] = out->cps_h[1] = 1;
     return false;
 }
 
 template <int KIND>
 static int launch_happly(lise_ctx* c, const HArgs& a)
 {
-    dim3 grid(KIND == 0 ? c->L.nx : c->L.ny, c->G);
+    HArgs b = a;
+    b.G = c->G * c->ks.cps_h[KIND];
+    dim3 grid(KIND == 0 ? c->L.nx : c->L.ny, b.G);
     prof_begin(c, KIND == 0 ? PC_HAPPLY_YZ : PC_HAPPLY_XZ);
-    (KIND == 0 ? c->ks.h_yz : c->ks.h_xz)<<<grid, c->ks.thr_h[KIND], c->ks.smem_h[KIND], c->stream>>>(a);
+    (KIND == 0 ? c->ks.h_yz : c->ks.h_xz)<<<grid, c->ks.thr_h[KIND], c->ks.smem_h[KIND], c->stream>>>(b);
     prof_end(c);
     CKL();
     return LISE_OK;
@@ -327,7 +356,7 @@ static int launch_update(lise_ctx* c, const UArgs& a, cudaStream_t st)
 {
     prof_begin(c, PC_UPDATE, st);
     if (c->ks.v5) {
-        const size_t slen = (size_t)4 * c->L.nxyz, per = (size_t)LISE_UPD_THREADS * LISE_UPD_EPT;
+        const size_t slen = (size_t)4 * c->L.nxyz, per = (size_t)LISE_UPD_THREADS * UpdEpt<MODE>::V;
         dim3 grid((unsigned)((slen + per - 1) / per), a.ns);
         c->ks.u[MODE]<<<grid, LISE_UPD_THREADS, 0, st>>>(a);
     } else {
@@ -424,6 +453,7 @@ static int dens_chunk(lise_ctx* c, int q, const cplx* Z, int ns)
 static int dens_accumulate(lise_ctx* c, int q, const cplx* Z)
 {
     const size_t slen = (size_t)4 * c->L.nxyz;
+    if (c->ks.v5) return c->nwf[q] > 0 ? dens_chunk(c, q, Z, c->nwf[q]) : LISE_OK;   // one launch pair per species
     for (int s0 = 0; s0 < c->nwf[q]; s0 += c->chunk) {
         const int ns = (c->nwf[q] - s0 < c->chunk) ? c->nwf[q] - s0 : c->chunk;
         TRY(dens_chunk(c, q, Z + s0 * slen, ns));
@@ -516,13 +546,23 @@ static int abm_step(lise_ctx* c)
     for (int phase = 1; phase <= 2; ++phase) {
         TRY(zero_partials(c, 0)); TRY(zero_partials(c, 1));
         int i = 0;                                  // chunk counter across both species
-        int pq = -1, pns = 0; size_t poff = 0;      // previous chunk: its densities are still to be accumulated
+        // densities of the new state: accumulated over groups of `dgroup` chunks (one launch pair per group), behind
+        // the H-apply of the following chunk so that the update of the last chunk of the group overlaps it
+        int pend_q = -1, pend_ns = 0, pend_chunks = 0; size_t pend_off = 0;
+        auto flush_dens = [&](int last_chunk) -> int {
+            if (pend_q < 0) return LISE_OK;
+            if (pipe) CK(cudaStreamWaitEvent(c->stream, c->ev_u[last_chunk & 1], 0));
+            TRY(dens_chunk(c, pend_q, (phase == 1 ? S(c, pend_q, RF) : S(c, pend_q, RB)) + pend_off, pend_ns));
+            pend_q = -1; pend_ns = 0; pend_chunks = 0;
+            return LISE_OK;
+        };
         for (int q = 0; q < 2; ++q)
             for (int s0 = 0; s0 < c->nwf[q]; s0 += c->chunk, ++i) {
                 const int ns = (c->nwf[q] - s0 < c->chunk) ? c->nwf[q] - s0 : c->chunk;
                 const size_t off = s0 * slen;
                 const int wb = pipe ? (i & 1) : 0;
                 const cplx* X = (phase == 1 ? S(c, q, RA) : S(c, q, RF)) + off;
+                if (pipe && i >= 2) CK(cudaStreamWaitEvent(c->stream, c->ev_u[wb], 0));   // W[wb], eta[wb] are free again
                 TRY(apply_h_chunk(c, q, X, Wbuf(c, wb), etabuf(c, wb), ns));
                 UArgs u = make_uargs(c, q, off, ns, wb);
                 cudaStream_t su = pipe ? c->stream2 : c->stream;
@@ -530,21 +570,14 @@ static int abm_step(lise_ctx* c)
                 if (phase == 1) TRY(launch_update<1>(c, u, su)); else TRY(launch_update<2>(c, u, su));
                 if (pipe) CK(cudaEventRecord(c->ev_u[wb], c->stream2));
                 if (c->ks.v5) {
-                    if (pipe) {
-                        if (pq >= 0) {              // densities of the previous chunk, behind this chunk's H-apply
-                            CK(cudaStreamWaitEvent(c->stream, c->ev_u[wb ^ 1], 0));
-                            TRY(dens_chunk(c, pq, (phase == 1 ? S(c, pq, RF) : S(c, pq, RB)) + poff, pns));
-                        }
-                        pq = q; pns = ns; poff = off;
-                    } else TRY(dens_chunk(c, q, (phase == 1 ? S(c, q, RF) : S(c, q, RB)) + off, ns));
+                    if (pend_q >= 0 && (pend_q != q || pend_chunks >= c->dgroup)) TRY(flush_dens(i - 1));
+                    if (pend_q < 0) { pend_q = q; pend_off = off; }
+                    pend_ns += ns; pend_chunks += 1;
                 } else {
                     TRY(launch_dens_x(c, make_dargs(c, q, (phase == 1 ? S(c, q, RF) : S(c, q, RB)) + off, ns)));
                 }
             }
-        if (pipe && pq >= 0) {
-            CK(cudaStreamWaitEvent(c->stream, c->ev_u[(i - 1) & 1], 0));
-            TRY(dens_chunk(c, pq, (phase == 1 ? S(c, pq, RF) : S(c, pq, RB)) + poff, pns));
-        }
+        TRY(flush_dens(i - 1));
         if (phase == 1) TRY(grid_phase(c, 1));     // potentials of the modifier m
     }
     // y_{n+1} sits in B: A <-> B; f history shifts
@@ -655,6 +688,7 @@ static int default_chunk(const lise_ctx* c)
     int ch = (int)(32.0 * 1048576.0 / sbytes);
     if (ch < c->G) ch = c->G;
     ch = (ch / c->G) * c->G;
+    if (const char* e = getenv("LISE_CHUNK")) { int v = atoi(e); if (v > 0) ch = v; }
     if (ch > nmax) ch = nmax;
     if (ch < 1) ch = 1;
     return ch;
@@ -732,6 +766,8 @@ static int ctx_init(lise_ctx* c)
     }
     c->overlap = 1;
     if (const char* e = getenv("LISE_OVERLAP")) c->overlap = atoi(e) ? 1 : 0;
+    c->dgroup = 8;
+    if (const char* e = getenv("LISE_DGROUP")) { int g = atoi(e); if (g > 0) c->dgroup = g; }
     // state slots and scratch
     for (int q = 0; q < 2; ++q)
         for (int s = 0; s < LISE_NSLOT; ++s) {

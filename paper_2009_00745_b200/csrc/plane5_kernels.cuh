@@ -26,6 +26,28 @@ __device__ __forceinline__ void bar_named(int id, int nthreads)
 
 // 8-byte part (re if !im, im if im) of a complex in shared memory
 __device__ __forceinline__ double ld_part(const cplx* p, int idx, bool im) { return ((const double*)p)[2 * idx + (im ? 1 : 0)]; }
+// x with its sign bit xor-ed by sgn (0 or 0x80000000): conjugation on the integer pipe, the fp64 pipe stays free
+__device__ __forceinline__ double xor_sign(double x, unsigned sgn) { return __hiloint2double(__double2hiint(x) ^ (int)sgn, __double2loint(x)); }
+
+// -i B a for the 2x2 Hermitian B = A + (sigma x W)_axis / 2 (compact potentials A, w1, w2 of AxisPot4), per axis
+template <int AXIS>
+__device__ __forceinline__ void apply_miB(double A, double w1, double w2, cplx au, cplx ad, cplx& ou, cplx& od)
+{
+    double tur, tui, tdr, tdi;
+    if (AXIS == 0) {            // b00 = A - w1, b11 = A + w1, b01 = (0, beta), beta = -w2
+        const double b00 = A - w1, b11 = A + w1;
+        tur = fma(b00, au.x, w2 * ad.y);  tui = fma(b00, au.y, -w2 * ad.x);
+        tdr = fma(b11, ad.x, -w2 * au.y); tdi = fma(b11, ad.y, w2 * au.x);
+    } else if (AXIS == 1) {     // b00 = A + w1, b11 = A - w1, b01 = (alpha, 0), alpha = -w2
+        const double b00 = A + w1, b11 = A - w1;
+        tur = fma(b00, au.x, -w2 * ad.x); tui = fma(b00, au.y, -w2 * ad.y);
+        tdr = fma(b11, ad.x, -w2 * au.x); tdi = fma(b11, ad.y, -w2 * au.y);
+    } else {                    // b00 = b11 = A, b01 = (w1, w2)
+        tur = fma(A, au.x, fma(w1, ad.x, -w2 * ad.y)); tui = fma(A, au.y, fma(w1, ad.y, w2 * ad.x));
+        tdr = fma(A, ad.x, fma(w1, au.x, w2 * au.y));  tdi = fma(A, ad.y, fma(w1, au.y, -w2 * au.x));
+    }
+    ou = cmk(tui, -tur); od = cmk(tdi, -tdr);
+}
 
 template <int N> struct TaskGeom {
     typedef LOp<N> L;
@@ -46,7 +68,7 @@ __device__ __forceinline__ void taxis_core5(const cplx* __restrict__ phi_u, cons
     constexpr bool SPLIT = (R * NTH >= 6);        // long lines: one operator at a time (register budget)
     const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
     const bool im = g & 1;
-    const double cs = (CONJ && im) ? -1.0 : 1.0;  // sign of this lane's part under conjugation
+    const unsigned cs = (CONJ && im) ? 0x80000000u : 0u;   // sign flip of this lane's part under conjugation
     const int ibase = (l0 + (g >> 1)) * LS + t * PS;
     const int obase = (l0 + t) * LS + g * PS;
     // ---- phase 1: a = D phi, b = D2 phi; result = -i B a - M b / 2 ----
@@ -64,7 +86,8 @@ __device__ __forceinline__ void taxis_core5(const cplx* __restrict__ phi_u, cons
 #pragma unroll
                 for (int m = 0; m < R; ++m) {
                     const int ii = ibase + (H * m + 4 * kk) * PS;
-                    xu[m] = cs * ld_part(phi_u, ii, im); xd[m] = cs * ld_part(phi_d, ii, im);
+                    xu[m] = ld_part(phi_u, ii, im); xd[m] = ld_part(phi_d, ii, im);
+                    if (CONJ) { xu[m] = xor_sign(xu[m], cs); xd[m] = xor_sign(xd[m], cs); }
                 }
                 RDFT<R>::fwd(xu, vu); RDFT<R>::fwd(xd, vd);
                 if (!SPLIT || op == 0) { mma_blocks<N>(au, F1, vu, kk); mma_blocks<N>(ad, F1, vd, kk); }
@@ -79,13 +102,11 @@ __device__ __forceinline__ void taxis_core5(const cplx* __restrict__ phi_u, cons
                 const int idx = m * NTH + r;
                 if (8 * r + g >= H) { ru[idx] = cmk(0.0, 0.0); rd[idx] = cmk(0.0, 0.0); continue; }   // padding rows
                 const int oi = obase + (H * m + 8 * r) * PS;
-                const double M = pot.M[oi];
-                double b00, b11, br, bi;
-                make_B4<AXIS>(pot.A[oi], pot.w1[oi], pot.w2[oi], b00, b11, br, bi);
+                const double mh = pot.M[oi];                                       // -M / 2
                 cplx lu, ld_;
-                apply_C(b00, b11, cmk(br, bi), cmk(au[m][r][0], au[m][r][1]), cmk(ad[m][r][0], ad[m][r][1]), lu, ld_);   // -i B D phi
-                ru[idx] = cmk(fma(-0.5 * M, bu[m][r][0], lu.x), fma(-0.5 * M, bu[m][r][1], lu.y));
-                rd[idx] = cmk(fma(-0.5 * M, bd[m][r][0], ld_.x), fma(-0.5 * M, bd[m][r][1], ld_.y));
+                apply_miB<AXIS>(pot.A[oi], pot.w1[oi], pot.w2[oi], cmk(au[m][r][0], au[m][r][1]), cmk(ad[m][r][0], ad[m][r][1]), lu, ld_);   // -i B D phi
+                ru[idx] = cmk(fma(mh, bu[m][r][0], lu.x), fma(mh, bu[m][r][1], lu.y));
+                rd[idx] = cmk(fma(mh, bd[m][r][0], ld_.x), fma(mh, bd[m][r][1], ld_.y));
             }
     }
     // ---- phase 2: c = D g + D2 q,  g = -i B phi,  q = -M phi / 2 ----
@@ -104,11 +125,10 @@ __device__ __forceinline__ void taxis_core5(const cplx* __restrict__ phi_u, cons
                 for (int m = 0; m < R; ++m) {
                     const int ii = ibase + (H * m + 4 * kk) * PS;
                     cplx fu = phi_u[ii], fd = phi_d[ii];
-                    if (CONJ) { fu.y = -fu.y; fd.y = -fd.y; }
-                    const double M = pot.M[ii];
+                    if (CONJ) { fu.y = xor_sign(fu.y, 0x80000000u); fd.y = xor_sign(fd.y, 0x80000000u); }
                     if (!SPLIT || op == 0) g_part4<AXIS>(im, pot.A[ii], pot.w1[ii], pot.w2[ii], fu, fd, gu[m], gd[m]);
                     if (!SPLIT || op == 1) {
-                        const double mh = -0.5 * M;
+                        const double mh = pot.M[ii];                                   // -M / 2
                         qu[m] = mh * (im ? fu.y : fu.x); qd[m] = mh * (im ? fd.y : fd.x);
                     }
                 }
@@ -143,8 +163,8 @@ __device__ __forceinline__ void taxis_core5(const cplx* __restrict__ phi_u, cons
 // epilogue adds the y result, V_loc phi, the pairing block, maps the v pair back (-conj) and stores W to global.
 // shared: tables | phi[NBUF][NCOMP][PP] | out[NCOMP][PP] | pots M, Ay, Az, hWx, hWy, hWz [PP] | pV[6][PP] (VSTAGE)
 // ------------------------------------------------------------------------------------------------
-template <int NY, int NZ, int NCOMP, int NBUF, int NWARP, bool VSTAGE>
-__global__ void __launch_bounds__(NWARP * 32, 1) k5_happly_yz(HArgs a)
+template <int NY, int NZ, int NCOMP, int NBUF, int NWARP, bool VSTAGE, int MAXR>
+__global__ void __maxnreg__(MAXR) k5_happly_yz(HArgs a)
 {
     extern __shared__ double2 smem[];
     constexpr int LD = ldpad(NZ), PP = NY * LD, NPTS = NY * NZ;
@@ -165,7 +185,7 @@ __global__ void __launch_bounds__(NWARP * 32, 1) k5_happly_yz(HArgs a)
     for (int i = threadIdx.x; i < LOp<NZ>::TABSZ; i += blockDim.x) s_tz[i] = a.stab[2][i];
     for (int p = threadIdx.x; p < NPTS; p += blockDim.x) {
         const int y = p / NZ, z = p - y * NZ, si = y * LD + z, gi = gbase + p;
-        pM[si] = pot[(size_t)P_M * nxyz + gi];
+        pM[si] = -0.5 * pot[(size_t)P_M * nxyz + gi];
         pAy[si] = pot[(size_t)(P_A + 1) * nxyz + gi]; pAz[si] = pot[(size_t)(P_A + 2) * nxyz + gi];
         pWx[si] = 0.5 * pot[(size_t)(P_W + 0) * nxyz + gi]; pWy[si] = 0.5 * pot[(size_t)(P_W + 1) * nxyz + gi];
         pWz[si] = 0.5 * pot[(size_t)(P_W + 2) * nxyz + gi];
@@ -276,8 +296,8 @@ __global__ void __launch_bounds__(NWARP * 32, 1) k5_happly_yz(HArgs a)
 // before the DMMA passes and consumed in the epilogue.
 // shared: table | phi[NBUF][NCOMP][PP] | pots M, Ax, hWy, hWz [PP] | red[2][NWARP]
 // ------------------------------------------------------------------------------------------------
-template <int NX, int NZ, int NCOMP, int NBUF, int NWARP>
-__global__ void __launch_bounds__(NWARP * 32, 1) k5_happly_xz(HArgs a)
+template <int NX, int NZ, int NCOMP, int NBUF, int NWARP, int MAXR>
+__global__ void __maxnreg__(MAXR) k5_happly_xz(HArgs a)
 {
     extern __shared__ double2 smem[];
     constexpr int LD = ldpad(NZ), PP = NX * LD, NPTS = NX * NZ;
@@ -294,7 +314,7 @@ __global__ void __launch_bounds__(NWARP * 32, 1) k5_happly_xz(HArgs a)
     for (int i = threadIdx.x; i < L::TABSZ; i += blockDim.x) s_tx[i] = a.stab[0][i];
     for (int p = threadIdx.x; p < NPTS; p += blockDim.x) {
         const int x = p / NZ, z = p - x * NZ, si = x * LD + z, gi = gb + x * gs + z;
-        pM[si] = pot[(size_t)P_M * nxyz + gi];
+        pM[si] = -0.5 * pot[(size_t)P_M * nxyz + gi];
         pAx[si] = pot[(size_t)(P_A + 0) * nxyz + gi];
         pWy[si] = 0.5 * pot[(size_t)(P_W + 1) * nxyz + gi]; pWz[si] = 0.5 * pot[(size_t)(P_W + 2) * nxyz + gi];
     }
@@ -383,8 +403,10 @@ __global__ void __launch_bounds__(NWARP * 32, 1) k5_happly_xz(HArgs a)
 //   MODE 3 (starter, Taylor term `order`): as k_update_yz<3> in state_kernels.cuh
 // History slots are read and written with streaming cache hints so that W, X and the new state stay in L2.
 // ------------------------------------------------------------------------------------------------
-#define LISE_UPD_THREADS 256
-#define LISE_UPD_EPT 2
+// 128 threads and <= 128 registers: one CTA fits beside a 12-warp, 128-register H-apply CTA on the same SM, so the
+// update of chunk i streams from HBM while the tensor-core kernels of chunk i + 1 run.
+#define LISE_UPD_THREADS 128
+template <int MODE> struct UpdEpt { static constexpr int V = (MODE == 1) ? 3 : (MODE == 2) ? 6 : 2; };   // elements per thread
 template <int MODE>
 __global__ void __launch_bounds__(LISE_UPD_THREADS) k5_update(UArgs a)
 {
@@ -405,6 +427,7 @@ __global__ void __launch_bounds__(LISE_UPD_THREADS) k5_update(UArgs a)
     const double eta = s_eta;
     const double ih = 1.0 / a.hbarc, c48 = a.dt / 48.0;
     const size_t so = (size_t)st * slen;
+    constexpr int LISE_UPD_EPT = UpdEpt<MODE>::V;
     const size_t e0 = (size_t)blockIdx.x * (LISE_UPD_THREADS * LISE_UPD_EPT) + threadIdx.x;
     if (MODE == 1) {
         cplx w[LISE_UPD_EPT], y[LISE_UPD_EPT], ym[LISE_UPD_EPT], f1[LISE_UPD_EPT], f2[LISE_UPD_EPT], f3[LISE_UPD_EPT], e[LISE_UPD_EPT];
@@ -487,7 +510,7 @@ __device__ __forceinline__ void dens_axis_task5(const cplx* __restrict__ v_u, co
     constexpr int R = L::R, NTH = L::NTH, NKH = L::NKH, H = L::H;
     const int lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
     const bool im = g & 1;
-    const double cs = im ? -1.0 : 1.0;                      // phi = conj(v)
+    const unsigned cs = im ? 0x80000000u : 0u;              // phi = conj(v)
     const int ibase = (l0 + (g >> 1)) * LS + t * PS;
     const int obase = (l0 + t) * LS + g * PS;
     Frags<N> F;
@@ -500,7 +523,7 @@ __device__ __forceinline__ void dens_axis_task5(const cplx* __restrict__ v_u, co
 #pragma unroll
         for (int m = 0; m < R; ++m) {
             const int ii = ibase + (H * m + 4 * kk) * PS;
-            xu[m] = cs * ld_part(v_u, ii, im); xd[m] = cs * ld_part(v_d, ii, im);
+            xu[m] = xor_sign(ld_part(v_u, ii, im), cs); xd[m] = xor_sign(ld_part(v_d, ii, im), cs);
         }
         RDFT<R>::fwd(xu, vu); RDFT<R>::fwd(xd, vd);
         mma_blocks<N>(au, F, vu, kk); mma_blocks<N>(ad, F, vd, kk);

@@ -28,7 +28,7 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 //                                   y: b00 = A + hWx, b11 = A - hWx, b01 = (-hWz, 0)
 //                                   z: b00 = b11 = A,               b01 = (hWy, hWx)        (hW = W / 2)
 struct AxisPot4 {
-    const double* M;      // hbar^2 / 2m*
+    const double* M;      // -(hbar^2 / 2m*) / 2
     const double* A;      // A_axis
     const double* w1;     // x: hWy   y: hWx   z: hWy
     const double* w2;     // x: hWz   y: hWz   z: hWx
