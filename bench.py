@@ -212,10 +212,14 @@ def run_ours(args):
     obs = g.observables()
 
     # ---- per-kernel-class device times (CUDA events inside the library, on the launching stream) ----
+    # with the two-stream overlap off: a class time is then that kernel running alone, which is what a per-kernel
+    # roofline needs (overlapped, the update and the H-apply kernels share SMs and stretch each other)
+    g.set_overlap(False)
     g.profile(True)
     g.step(max(1, min(args.steps, 2)))
     prof = g.profile_read()
     g.profile(False)
+    g.set_overlap(os.environ.get("LISE_OVERLAP", "1") != "0")
     psteps = max(1, min(args.steps, 2))
 
     # ---- end to end through the C-ABI with HOST buffers ----
@@ -276,6 +280,7 @@ def run_ours(args):
     roof["share_of_step"] = top_ms / tot_ms if tot_ms > 0 else None
     roof["traffic"] = None
     roof["classes_ms_per_step"] = {k: v[0] / psteps for k, v in prof.items()}
+    roof["classes_note"] = "per-class device time with the update/H-apply stream overlap off; the timed region runs with it on"
     step_bytes = 15.0 * S                                              # B_min = 960 Nxyz per qpwf-update
     per_gpu = value / world
     step_roof = {"hbm_bytes_per_update": step_bytes, "hbm_frac_of_measured": per_gpu * step_bytes / (hbm_gbs * 1e9),

@@ -150,10 +150,27 @@ int lise_profile_read(lise_ctx *ctx, double *ms, long *counts);
  * (HOST pointer).  sm_mhz_host is reserved (set to 0).  Synchronises. */
 int lise_measure_fp64_peak(void *stream, double seconds, double *tflops_host, double *sm_mhz_host);
 
+/* Microbenchmark behind DESIGN.md's fp64-pipe model: every warp of a 1-CTA-per-SM grid with `warps` warps loops over
+ * a bundle of independent m8n8k4 DMMAs and DFMAs (variant 0: 8 DMMA, 1: 16 DFMA, 2: 8 + 8, 3: 8 + 16, 4: 8 + 32,
+ * 5: 16 DMMA); writes the SM clocks one bundle iteration takes (wall time x nominal SM clock / iterations) to
+ * *clocks_per_iter_host (HOST).  Synchronises; uses the default stream. */
+int lise_measure_fp64_mix(int variant, int warps, double *clocks_per_iter_host);
+
 /* Which line operator the per-state kernels of this context use: "dmma" (fp64 tensor-core tiles, for the
  * lattice shapes the library was instantiated for; LISE_LINE_OP=dense in the environment disables it)
  * or "dense" (generic DFMA circulant sums, any even lattice).  Both apply the same operator (Eq. 48). */
 const char *lise_line_operator(const lise_ctx *ctx);
+
+/* Host-only (no CUDA call, works without a GPU): the block-diagonalised form of the lattice derivative matrices
+ * D (Eq. 48a) and D2 (Eq. 48b, prefactor as DESIGN.md B3) of a periodic line of n points (n % 4 == 0) that the
+ * tensor-core kernels use.  dims_host (HOST, 5 ints) receives H (block size), R = n / H, J = R / 2 + 1 (blocks),
+ * ND (entries per Toeplitz table) and the table length; tab_host (HOST, may be NULL to query the sizes, else at
+ * least dims[4] doubles as stated by cap) receives tab[((op * J + j) * 2 + pq) * ND + d + H - 1] with op = 0 (D),
+ * 1 (D2), pq = 0 (P_j), 1 (Q_j), d = r - r' in (-H, H):
+ *   P_j[d] = (w_j / R) sum_p cos(2 pi j p / R) c[(d + H p) mod n],  Q_j with sin,  w_j = 1 for j = 0, R/2, else 2,
+ * so that with b_j = sum_m cos(2 pi j m / R) x[r' + H m], e_j likewise with sin, S_j = P_j b_j - Q_j e_j,
+ * T_j = P_j e_j + Q_j b_j:  (C x)[r + H m] = sum_j cos(2 pi j m / R) S_j[r] + sin(2 pi j m / R) T_j[r]. */
+int lise_line_operator_tables(int n, double dx, double *tab_host, int cap, int *dims_host);
 
 /* Number of kernel launches issued by this context so far (for bench.py's gpu_launches). */
 long lise_launch_count(const lise_ctx *ctx);

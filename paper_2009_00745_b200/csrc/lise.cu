@@ -250,9 +250,9 @@ static constexpr size_t v5_smem_happly_yz(int ncomp, int nbuf, bool vstage)
          + 8 * (size_t)(NY * ldpad(NZ)) * (6 + (vstage ? 6 : 0));
 }
 template <int NX, int NZ>
-static constexpr size_t v5_smem_happly_xz(int ncomp, int nbuf, int nwarp)
+static constexpr size_t v5_smem_happly_xz(int ncomp, int nbuf, int nwarp, bool wst = false)
 {
-    return 8 * ((tabsz<NX>() + 1) / 2 * 2) + 16 * (size_t)(NX * ldpad(NZ)) * ncomp * nbuf + 8 * (size_t)(NX * ldpad(NZ)) * 4 + 8 * 2 * nwarp;
+    return 8 * ((tabsz<NX>() + 1) / 2 * 2) + 16 * (size_t)(NX * ldpad(NZ)) * ncomp * nbuf * (wst ? 2 : 1) + 8 * (size_t)(NX * ldpad(NZ)) * 4 + 8 * 2 * nwarp;
 }
 template <int NY, int NZ>
 static constexpr size_t v5_smem_dens_yz() { return 8 * ((tabsz<NY>() + tabsz<NZ>() + 1) / 2 * 2) + 16 * (size_t)(4 * NY * ldpad(NZ)); }
@@ -302,13 +302,14 @@ static KernSet make_v5_set()
     KernSet k;
     // register caps: 128 where a 12-warp CTA then leaves room for one update CTA per SM (overlap), else what fits
     constexpr int RYZ = TWO_YZ ? v5_maxr(WYZ, 2) : v5_maxr(WYZ, 1), RXZ = TWO_XZ ? v5_maxr(WXZ, 2) : v5_maxr(WXZ, 1);
-    k.h_yz = k5_happly_yz<NY, NZ, CYZ, BYZ, WYZ, VST, RYZ>; k.h_xz = k5_happly_xz<NX, NZ, CXZ, BXZ, WXZ, RXZ>;
+    constexpr bool WST = !TWO_XZ && BXZ == 2 && v5_smem_happly_xz<NX, NZ>(CXZ, BXZ, WXZ, true) <= SMEM_LIMIT;
+    k.h_yz = k5_happly_yz<NY, NZ, CYZ, BYZ, WYZ, VST, RYZ>; k.h_xz = k5_happly_xz<NX, NZ, CXZ, BXZ, WXZ, RXZ, WST>;
     k.cps_h[0] = TWO_YZ ? 2 : 1; k.cps_h[1] = TWO_XZ ? 2 : 1;
     k.u[0] = nullptr; k.u[1] = k5_update<1>; k.u[2] = k5_update<2>; k.u[3] = k5_update<3>;
     k.d_yz = k5_dens_yz<NY, NZ, WDY>; k.d_x = k5_dens_x<NX, NZ, WDX>;
     k.name = "dmma"; k.v5 = 1;
     k.thr_h[0] = 32 * WYZ; k.thr_h[1] = 32 * WXZ; k.thr_u = LISE_UPD_THREADS; k.thr_d = 32 * WDX; k.thr_dyz = 32 * WDY;
-    k.smem_h[0] = v5_smem_happly_yz<NY, NZ>(CYZ, BYZ, VST); k.smem_h[1] = v5_smem_happly_xz<NX, NZ>(CXZ, BXZ, WXZ);
+    k.smem_h[0] = v5_smem_happly_yz<NY, NZ>(CYZ, BYZ, VST); k.smem_h[1] = v5_smem_happly_xz<NX, NZ>(CXZ, BXZ, WXZ, WST);
     k.smem_u = 0; k.smem_d = v5_smem_dens_x<NX, NZ>(); k.smem_dyz = v5_smem_dens_yz<NY, NZ>();
     k.ups_xz = 4 / CXZ;
     return k;
@@ -1082,6 +1083,54 @@ extern "C" int lise_measure_fp64_peak(void* stream, double seconds, double* tflo
     *tflops_host = best;
     if (sm_mhz_host) *sm_mhz_host = 0.0;
     return rc;
+}
+
+// clocks per iteration and SM sub-partition of the DMMA/DFMA mix `variant` with `warps` warps per CTA (1 CTA per SM)
+extern "C" int lise_measure_fp64_mix(int variant, int warps, double* clocks_per_iter_host)
+{
+    if (!clocks_per_iter_host || warps < 1 || warps > 12) return LISE_EINVAL;
+    int dev = 0, nsm = 0, khz = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return LISE_ECUDA;
+    cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, dev);
+    double* out = nullptr;
+    if (cudaMalloc(&out, sizeof(double) * nsm * 384) != cudaSuccess) return LISE_ENOMEM;
+    cudaEvent_t e0, e1; cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int iters = 20000;
+    float best = 1e30f;
+    for (int rep = 0; rep < 4; ++rep) {
+        cudaEventRecord(e0, 0);
+        switch (variant) {
+        case 0: k_fp64_mix<8, 0><<<nsm, 32 * warps>>>(out, iters, 0.999999, 1e-9); break;
+        case 1: k_fp64_mix<0, 16><<<nsm, 32 * warps>>>(out, iters, 0.999999, 1e-9); break;
+        case 2: k_fp64_mix<8, 8><<<nsm, 32 * warps>>>(out, iters, 0.999999, 1e-9); break;
+        case 3: k_fp64_mix<8, 16><<<nsm, 32 * warps>>>(out, iters, 0.999999, 1e-9); break;
+        case 4: k_fp64_mix<8, 32><<<nsm, 32 * warps>>>(out, iters, 0.999999, 1e-9); break;
+        case 5: k_fp64_mix<16, 0><<<nsm, 32 * warps>>>(out, iters, 0.999999, 1e-9); break;
+        default: cudaFree(out); return LISE_EINVAL;
+        }
+        cudaEventRecord(e1, 0);
+        if (cudaEventSynchronize(e1) != cudaSuccess || cudaGetLastError() != cudaSuccess) { cudaFree(out); return LISE_ECUDA; }
+        float ms = 0.f; cudaEventElapsedTime(&ms, e0, e1);
+        if (ms < best) best = ms;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(out);
+    // warps are spread over the 4 sub-partitions: clocks per iteration of ONE warp's instruction bundle, per sub-partition share
+    *clocks_per_iter_host = (double)best * 1e-3 * (double)khz * 1e3 / iters;
+    return LISE_OK;
+}
+
+// host-only: the block-diagonalised tables of a line of n points (no CUDA call; tests pin them against Eqs. 49-50)
+extern "C" int lise_line_operator_tables(int n, double dx, double* tab_host, int cap, int* dims_host)
+{
+    if (n < 4 || n % 4 != 0 || !(dx > 0.0) || !dims_host) return LISE_EINVAL;
+    const LOpDims D = lop_dims(n);
+    dims_host[0] = D.H; dims_host[1] = D.R; dims_host[2] = D.J; dims_host[3] = D.ND; dims_host[4] = D.TABSZ;
+    if (!tab_host) return LISE_OK;
+    if (cap < D.TABSZ) return LISE_EINVAL;
+    std::vector<double> t;
+    host_stab(n, dx, t);
+    memcpy(tab_host, t.data(), sizeof(double) * t.size());
+    return LISE_OK;
 }
 
 extern "C" const char* lise_line_operator(const lise_ctx* c) { return c ? c->ks.name : "none"; }

@@ -183,6 +183,7 @@ __global__ void __maxnreg__(MAXR) k5_happly_yz(HArgs a)
     const double* pot = a.pot;
     for (int i = threadIdx.x; i < LOp<NY>::TABSZ; i += blockDim.x) s_ty[i] = a.stab[1][i];
     for (int i = threadIdx.x; i < LOp<NZ>::TABSZ; i += blockDim.x) s_tz[i] = a.stab[2][i];
+    auto stage_pots = [&]() {
     for (int p = threadIdx.x; p < NPTS; p += blockDim.x) {
         const int y = p / NZ, z = p - y * NZ, si = y * LD + z, gi = gbase + p;
         pM[si] = -0.5 * pot[(size_t)P_M * nxyz + gi];
@@ -195,6 +196,7 @@ __global__ void __maxnreg__(MAXR) k5_happly_yz(HArgs a)
             for (int k = 0; k < 6; ++k) pV[k * PP + si] = v[k];
         }
     }
+    };
     const AxisPot4 poty = {pM, pAy, pWx, pWz}, potz = {pM, pAz, pWy, pWx};
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
     const int pr = warp / WPP, lw = warp - pr * WPP;        // this warp's pair (within the unit) and index in it
@@ -213,6 +215,7 @@ __global__ void __maxnreg__(MAXR) k5_happly_yz(HArgs a)
 
     int u = blockIdx.y;
     if (u < nunits) issue(u, 0);
+    stage_pots();                                           // behind the first prefetch
     for (int it = 0; u < nunits; u += a.G, ++it) {
         const int buf = (NBUF == 2) ? (it & 1) : 0;
         cp_async_wait<0>();
@@ -294,9 +297,9 @@ __global__ void __maxnreg__(MAXR) k5_happly_yz(HArgs a)
 // H-apply, xz-planes:  W += T_x X,  eta_part[(st * UPS + pg) * ny + iy] = dV Re <X|W> over the plane.
 // grid (ny, G), NWARP warps.  One barrier per unit; the W values of a thread's output points are read from global
 // before the DMMA passes and consumed in the epilogue.
-// shared: table | phi[NBUF][NCOMP][PP] | pots M, Ax, hWy, hWz [PP] | red[2][NWARP]
+// shared: table | phi[NBUF][NCOMP][PP] | w[NBUF][NCOMP][PP] (WST) | pots M, Ax, hWy, hWz [PP] | red[2][NWARP]
 // ------------------------------------------------------------------------------------------------
-template <int NX, int NZ, int NCOMP, int NBUF, int NWARP, int MAXR>
+template <int NX, int NZ, int NCOMP, int NBUF, int NWARP, int MAXR, bool WST>
 __global__ void __maxnreg__(MAXR) k5_happly_xz(HArgs a)
 {
     extern __shared__ double2 smem[];
@@ -307,17 +310,20 @@ __global__ void __maxnreg__(MAXR) k5_happly_xz(HArgs a)
     const int nxyz = a.L.nxyz, gs = a.L.ny * NZ, gb = blockIdx.x * NZ;
     double* s_tx = (double*)smem;
     cplx* phi = (cplx*)(s_tx + L::TABSZ + (L::TABSZ & 1));
-    double* pM = (double*)(phi + NBUF * NCOMP * PP);
+    cplx* wpl = phi + NBUF * NCOMP * PP;                    // WST: the unit's W plane, prefetched with its X plane
+    double* pM = (double*)(wpl + (WST ? NBUF * NCOMP * PP : 0));
     double *pAx = pM + PP, *pWy = pAx + PP, *pWz = pWy + PP;
     double* s_red = pWz + PP;                               // [2][NWARP]
     const double* pot = a.pot;
     for (int i = threadIdx.x; i < L::TABSZ; i += blockDim.x) s_tx[i] = a.stab[0][i];
+    auto stage_pots = [&]() {
     for (int p = threadIdx.x; p < NPTS; p += blockDim.x) {
         const int x = p / NZ, z = p - x * NZ, si = x * LD + z, gi = gb + x * gs + z;
         pM[si] = -0.5 * pot[(size_t)P_M * nxyz + gi];
         pAx[si] = pot[(size_t)(P_A + 0) * nxyz + gi];
         pWy[si] = 0.5 * pot[(size_t)(P_W + 1) * nxyz + gi]; pWz[si] = 0.5 * pot[(size_t)(P_W + 2) * nxyz + gi];
     }
+    };
     const AxisPot4 potx = {pM, pAx, pWy, pWz};
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
     const int nunits = a.ns * UPS;
@@ -326,9 +332,12 @@ __global__ void __maxnreg__(MAXR) k5_happly_xz(HArgs a)
         const int st = u / UPS, pg = u - st * UPS;
         const size_t go = ((size_t)st * 4 + pg * NCOMP) * nxyz + gb;
         cplx* dphi = phi + buf * NCOMP * PP;
+        cplx* dw = wpl + buf * NCOMP * PP;
         for (int i = threadIdx.x; i < NCOMP * NPTS; i += blockDim.x) {
             const int c = i / NPTS, p = i - c * NPTS, x = p / NZ, z = p - x * NZ;
-            cp_async16(dphi + c * PP + x * LD + z, a.X + go + (size_t)c * nxyz + (size_t)x * gs + z);
+            const size_t gi = go + (size_t)c * nxyz + (size_t)x * gs + z;
+            cp_async16(dphi + c * PP + x * LD + z, a.X + gi);
+            if (WST) cp_async16(dw + c * PP + x * LD + z, a.W + gi);
         }
         cp_async_commit();
     };
@@ -341,6 +350,7 @@ __global__ void __maxnreg__(MAXR) k5_happly_xz(HArgs a)
 
     int u = blockIdx.y, uprev = -1;
     if (u < nunits) issue(u, 0);
+    stage_pots();                                           // behind the first prefetch
     int it = 0;
     for (; u < nunits; u += a.G, ++it) {
         const int buf = (NBUF == 2) ? (it & 1) : 0;
@@ -358,16 +368,19 @@ __global__ void __maxnreg__(MAXR) k5_happly_xz(HArgs a)
             const cplx *fu = phib + 2 * pr * PP, *fd = fu + PP;
             cplx* Wu = a.W + ((size_t)st * 4 + 2 * pair) * nxyz + gb;
             cplx* Wd = Wu + nxyz;
-            cplx wu[NA], wd[NA];
+            const cplx *swu = wpl + (buf * NCOMP + 2 * pr) * PP, *swd = swu + PP;
+            cplx wu[WST ? 1 : NA], wd[WST ? 1 : NA];
+            if (!WST) {
 #pragma unroll
-            for (int m = 0; m < L::R; ++m)
+                for (int m = 0; m < L::R; ++m)
 #pragma unroll
-                for (int r = 0; r < L::NTH; ++r) {
-                    const int idx = m * L::NTH + r;
-                    if (8 * r + g >= L::H) { wu[idx] = cmk(0.0, 0.0); wd[idx] = cmk(0.0, 0.0); continue; }
-                    const size_t go = (size_t)(L::H * m + 8 * r + g) * gs + (l0 + t);
-                    wu[idx] = Wu[go]; wd[idx] = Wd[go];
-                }
+                    for (int r = 0; r < L::NTH; ++r) {
+                        const int idx = m * L::NTH + r;
+                        if (8 * r + g >= L::H) { wu[idx] = cmk(0.0, 0.0); wd[idx] = cmk(0.0, 0.0); continue; }
+                        const size_t go = (size_t)(L::H * m + 8 * r + g) * gs + (l0 + t);
+                        wu[idx] = Wu[go]; wd[idx] = Wd[go];
+                    }
+            }
             cplx ru[NA], rd[NA];
             if (pair) taxis_core5<NX, 0, true>(fu, fd, potx, l0, 1, LD, s_tx, ru, rd);
             else      taxis_core5<NX, 0, false>(fu, fd, potx, l0, 1, LD, s_tx, ru, rd);
@@ -378,7 +391,7 @@ __global__ void __maxnreg__(MAXR) k5_happly_xz(HArgs a)
                     const int idx = m * L::NTH + r;
                     if (8 * r + g >= L::H) continue;
                     const int x = L::H * m + 8 * r + g, z = l0 + t;
-                    cplx fu_ = wu[idx], fd_ = wd[idx];
+                    cplx fu_ = WST ? swu[x * LD + z] : wu[idx], fd_ = WST ? swd[x * LD + z] : wd[idx];
                     if (pair) { fu_ = cmk(fu_.x - ru[idx].x, fu_.y + ru[idx].y); fd_ = cmk(fd_.x - rd[idx].x, fd_.y + rd[idx].y); }
                     else      { fu_ = cadd(fu_, ru[idx]); fd_ = cadd(fd_, rd[idx]); }
                     const size_t go = (size_t)x * gs + z;

@@ -32,7 +32,7 @@ EXPORTS = ["lise_default_params", "lise_create", "lise_destroy", "lise_set_param
            "lise_set_dt", "lise_set_chunk", "lise_set_overlap", "lise_set_wavefunctions", "lise_get_wavefunctions",
            "lise_upload_wavefunctions", "lise_download_wavefunctions", "lise_set_reduce_hook",
            "lise_densities", "lise_potentials", "lise_apply_h", "lise_step", "lise_observables",
-           "lise_profile", "lise_profile_read", "lise_measure_fp64_peak", "lise_line_operator", "lise_launch_count", "lise_device_bytes", "lise_strerror", "lise_last_error"]
+           "lise_profile", "lise_profile_read", "lise_measure_fp64_peak", "lise_measure_fp64_mix", "lise_line_operator", "lise_line_operator_tables", "lise_launch_count", "lise_device_bytes", "lise_strerror", "lise_last_error"]
 
 
 REDUCE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_long)
@@ -84,6 +84,8 @@ def load():
     lib.lise_profile_read.argtypes = [vp, C.POINTER(dp), C.POINTER(C.c_long)]
     lib.lise_measure_fp64_peak.argtypes = [vp, dp, C.POINTER(dp), C.POINTER(dp)]
     lib.lise_line_operator.argtypes = [vp]; lib.lise_line_operator.restype = C.c_char_p
+    lib.lise_measure_fp64_mix.argtypes = [ip, ip, C.POINTER(dp)]
+    lib.lise_line_operator_tables.argtypes = [ip, dp, C.POINTER(dp), ip, C.POINTER(ip)]
     lib.lise_launch_count.argtypes = [vp]; lib.lise_launch_count.restype = C.c_long
     lib.lise_device_bytes.argtypes = [vp]; lib.lise_device_bytes.restype = C.c_longlong
     lib.lise_strerror.argtypes = [ip]; lib.lise_strerror.restype = C.c_char_p
@@ -108,6 +110,22 @@ def measure_fp64_peak(seconds=1.0, stream=None):
     if rc != 0:
         raise RuntimeError(f"lise_measure_fp64_peak failed ({rc})")
     return tf.value
+
+
+def line_operator_tables(n, dx):
+    """(dims dict, table as a numpy array [op][j][P|Q][d]) of the block-diagonalised line operator; host only."""
+    import numpy as np
+    lib = load()
+    dims = (C.c_int * 5)()
+    rc = lib.lise_line_operator_tables(n, dx, None, 0, dims)
+    if rc != 0:
+        raise RuntimeError(f"lise_line_operator_tables: {lib.lise_strerror(rc).decode()}")
+    H, R, J, ND, size = (int(v) for v in dims)
+    tab = np.zeros(size, dtype=np.float64)
+    rc = lib.lise_line_operator_tables(n, dx, tab.ctypes.data_as(C.POINTER(C.c_double)), size, dims)
+    if rc != 0:
+        raise RuntimeError(f"lise_line_operator_tables: {lib.lise_strerror(rc).decode()}")
+    return dict(H=H, R=R, J=J, ND=ND), tab.reshape(2, J, 2, ND)
 
 
 class LiseError(RuntimeError):
