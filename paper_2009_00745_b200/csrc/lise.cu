@@ -40,7 +40,11 @@ struct lise_ctx {
     cudaStream_t stream;
     double2* ctab[3];
     double* stab[3];                        // block-diagonalised line-operator tables (split_lineop.cuh)
-    cudaStream_t stream2;                   // the HBM-bound update kernels run here, overlapping the DMMA kernels
+    cudaStream_t stream2;                   // the HBM-bound update kernels run here (lowest priority), overlapping the DMMA kernels
+    cudaStream_t streamH;                   // highest priority: the DMMA kernels of lise_step run here when overlap is on, so
+                                            // that their CTAs are placed first and the update CTAs fill the room left beside them
+    cudaEvent_t ev_fork, ev_join;
+    cudaStream_t user_stream; int user_stream_valid;   // the caller's stream while lise_step runs on streamH
     cudaEvent_t ev_h[2], ev_u[2];
     int overlap, dgroup;                    // dgroup: chunks per density-kernel launch
     cplx* slot[2][LISE_NSLOT];
@@ -475,10 +479,14 @@ static int reduce_all(lise_ctx* c)
 {
     TRY(reduce_partials(c, 0)); TRY(reduce_partials(c, 1));
     if (c->reduce_fn) {
+        // the hook's contract names the CALLER's stream: bridge to it and back while the step runs on the internal one
+        const bool bridge = c->user_stream_valid && c->stream != c->user_stream;
+        if (bridge) { CK(cudaEventRecord(c->ev_fork, c->stream)); CK(cudaStreamWaitEvent(c->user_stream, c->ev_fork, 0)); }
         if (c->reduce_fn(c->reduce_user, c->acc[0], 2L * LISE_NACC * c->L.nxyz) != 0) {
             snprintf(c->err, sizeof(c->err), "reduce hook failed");
             return LISE_ECUDA;
         }
+        if (bridge) { CK(cudaEventRecord(c->ev_join, c->user_stream)); CK(cudaStreamWaitEvent(c->stream, c->ev_join, 0)); }
     }
     return LISE_OK;
 }
@@ -686,7 +694,7 @@ static int default_chunk(const lise_ctx* c)
 {
     const double sbytes = 64.0 * c->L.nxyz;
     int nmax = c->nwf[0] > c->nwf[1] ? c->nwf[0] : c->nwf[1];
-    int ch = (int)(32.0 * 1048576.0 / sbytes);
+    int ch = (int)(170.0 * 1048576.0 / sbytes);
     if (ch < c->G) ch = c->G;
     ch = (ch / c->G) * c->G;
     if (const char* e = getenv("LISE_CHUNK")) { int v = atoi(e); if (v > 0) ch = v; }
@@ -760,7 +768,14 @@ static int ctx_init(lise_ctx* c)
         CK(cudaMemcpy(c->stab[i], t.data(), sizeof(double) * t.size(), cudaMemcpyHostToDevice));
     }
     TRY(upload_rdft());
-    CK(cudaStreamCreateWithFlags(&c->stream2, cudaStreamNonBlocking));
+    {
+        int lo = 0, hi = 0;
+        CK(cudaDeviceGetStreamPriorityRange(&lo, &hi));
+        CK(cudaStreamCreateWithPriority(&c->stream2, cudaStreamNonBlocking, lo));
+        CK(cudaStreamCreateWithPriority(&c->streamH, cudaStreamNonBlocking, hi));
+        CK(cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
+        CK(cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming));
+    }
     for (int i = 0; i < 2; ++i) {
         CK(cudaEventCreateWithFlags(&c->ev_h[i], cudaEventDisableTiming));
         CK(cudaEventCreateWithFlags(&c->ev_u[i], cudaEventDisableTiming));
@@ -847,6 +862,9 @@ extern "C" void lise_destroy(lise_ctx* c)
     if (!c) return;
     cudaStreamSynchronize(c->stream);
     if (c->stream2) { cudaStreamSynchronize(c->stream2); cudaStreamDestroy(c->stream2); }
+    if (c->streamH) { cudaStreamSynchronize(c->streamH); cudaStreamDestroy(c->streamH); }
+    if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+    if (c->ev_join) cudaEventDestroy(c->ev_join);
     for (int i = 0; i < 2; ++i) { if (c->ev_h[i]) cudaEventDestroy(c->ev_h[i]); if (c->ev_u[i]) cudaEventDestroy(c->ev_u[i]); }
     if (c->allocs) {
         for (void* p : *c->allocs) cudaFree(p);
@@ -988,11 +1006,25 @@ extern "C" int lise_step(lise_ctx* c, int nsteps)
 {
     if (!c || nsteps < 0) return LISE_EINVAL;
     TRY(need_both(c));
-    for (int s = 0; s < nsteps; ++s) {
-        if (c->step < 3) TRY(starter_step(c)); else TRY(abm_step(c));
-        c->step += 1; c->time += c->dt;
+    // overlap on: fork from the caller's stream into the internal high-priority stream, join at the end
+    cudaStream_t user = c->stream;
+    const bool fork = c->ks.v5 && c->overlap && nsteps > 0;
+    if (fork) {
+        CK(cudaEventRecord(c->ev_fork, user));
+        CK(cudaStreamWaitEvent(c->streamH, c->ev_fork, 0));
+        c->stream = c->streamH; c->user_stream = user; c->user_stream_valid = 1;
     }
-    return LISE_OK;
+    int rc = LISE_OK;
+    for (int s = 0; s < nsteps && rc == LISE_OK; ++s) {
+        rc = (c->step < 3) ? starter_step(c) : abm_step(c);
+        if (rc == LISE_OK) { c->step += 1; c->time += c->dt; }
+    }
+    if (fork) {
+        c->stream = user; c->user_stream_valid = 0;
+        CK(cudaEventRecord(c->ev_join, c->streamH));
+        CK(cudaStreamWaitEvent(user, c->ev_join, 0));
+    }
+    return rc;
 }
 
 extern "C" int lise_observables(lise_ctx* c, lise_observables_t* o)
