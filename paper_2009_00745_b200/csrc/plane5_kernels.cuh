@@ -201,6 +201,21 @@ __global__ void __maxnreg__(MAXR) k5_happly_yz(HArgs a)
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
     const int pr = warp / WPP, lw = warp - pr * WPP;        // this warp's pair (within the unit) and index in it
     const int nunits = a.ns * UPS;
+    // ASYNC (two X buffers): no CTA-wide barrier inside the unit loop.  mbarriers F[buf] ("unit landed": every thread's
+    // cp.async copies arrive on it), E[buf] ("everyone is done with the unit in buf": out planes and X[buf] are free),
+    // Y[pair] ("the pair's y results are in the out planes").  Waits sit behind a DMMA pass, so warps drift by up to a
+    // task instead of stopping together.
+    constexpr bool ASYNC = (NBUF == 2);
+    __shared__ unsigned long long s_bar[6];
+    unsigned long long *barF = s_bar, *barE = s_bar + 2, *barY = s_bar + 4;
+    if (ASYNC) {
+        if (threadIdx.x == 0) {
+            mbar_init(barF, NWARP * 32); mbar_init(barF + 1, NWARP * 32);
+            mbar_init(barE, NWARP * 32); mbar_init(barE + 1, NWARP * 32);
+            mbar_init(barY, WPP * 32); mbar_init(barY + 1, WPP * 32);
+        }
+        __syncthreads();
+    }
 
     auto issue = [&](int u, int buf) {
         const int st = u / UPS, pg = u - st * UPS;
@@ -210,28 +225,36 @@ __global__ void __maxnreg__(MAXR) k5_happly_yz(HArgs a)
             const int c = i / NPTS, p = i - c * NPTS, y = p / NZ, z = p - y * NZ;
             cp_async16(dst + c * PP + y * LD + z, Xs + (size_t)c * nxyz + p);
         }
-        cp_async_commit();
+        if (ASYNC) mbar_arrive_cp_async(barF + buf); else cp_async_commit();
     };
 
     int u = blockIdx.y;
     if (u < nunits) issue(u, 0);
     stage_pots();                                           // behind the first prefetch
+    if (ASYNC) __syncthreads();                             // potentials and tables staged
     for (int it = 0; u < nunits; u += a.G, ++it) {
         const int buf = (NBUF == 2) ? (it & 1) : 0;
-        cp_async_wait<0>();
-        __syncthreads();                                    // unit u has landed; everyone is done with unit u - G
-        if (NBUF == 2 && u + a.G < nunits) issue(u + a.G, buf ^ 1);
+        if (ASYNC) mbar_wait(barF + buf, (it >> 1) & 1);    // unit u has landed
+        else { cp_async_wait<0>(); __syncthreads(); }       // ... and everyone is done with unit u - G
         const int st = u / UPS, pg = u - st * UPS;
         const int pair = pg * NPAIR + pr;                   // 0: u pair, 1: v pair
         const cplx* phib = phi + buf * NCOMP * PP;
         const cplx *fu = phib + 2 * pr * PP, *fd = fu + PP;
         cplx *ou = out + 2 * pr * PP, *od = ou + PP;
+        bool mid_done = false;
+        auto mid_unit = [&]() {                             // once per unit and thread, behind the first y pass
+            if (!ASYNC || mid_done) return;
+            mid_done = true;
+            if (it >= 1) mbar_wait(barE + (buf ^ 1), ((it - 1) >> 1) & 1);   // unit u - G: out planes and X[buf ^ 1] are free
+            if (u + a.G < nunits) issue(u + a.G, buf ^ 1);
+        };
         // ---- y lines (one per z): LS = 1, PS = LD; result -> out planes ----
         for (int task = lw; task < NZ / 4; task += WPP) {
             const int l0 = 4 * task;
             cplx ru[TaskGeom<NY>::NA], rd[TaskGeom<NY>::NA];
             if (pair) taxis_core5<NY, 1, true>(fu, fd, poty, l0, 1, LD, s_ty, ru, rd);
             else      taxis_core5<NY, 1, false>(fu, fd, poty, l0, 1, LD, s_ty, ru, rd);
+            mid_unit();
             typedef LOp<NY> L;
 #pragma unroll
             for (int m = 0; m < L::R; ++m)
@@ -242,7 +265,10 @@ __global__ void __maxnreg__(MAXR) k5_happly_yz(HArgs a)
                     ou[oi] = ru[m * L::NTH + r]; od[oi] = rd[m * L::NTH + r];
                 }
         }
-        bar_named(1 + pr, WPP * 32);                        // the pair's y results are complete
+        mid_unit();
+        if (ASYNC) mbar_arrive(barY + pr);                  // this thread's y results are in the out planes
+        else bar_named(1 + pr, WPP * 32);                   // the pair's y results are complete
+        bool y_waited = false;
         // ---- z lines (one per y): LS = LD, PS = 1; epilogue finishes W ----
         cplx* Ws = a.W + (size_t)st * 4 * nxyz;
         const cplx* Xst = a.X + (size_t)st * 4 * nxyz;
@@ -251,6 +277,7 @@ __global__ void __maxnreg__(MAXR) k5_happly_yz(HArgs a)
             cplx ru[TaskGeom<NZ>::NA], rd[TaskGeom<NZ>::NA];
             if (pair) taxis_core5<NZ, 2, true>(fu, fd, potz, l0, LD, 1, s_tz, ru, rd);
             else      taxis_core5<NZ, 2, false>(fu, fd, potz, l0, LD, 1, s_tz, ru, rd);
+            if (ASYNC && !y_waited) { mbar_wait(barY + pr, it & 1); y_waited = true; }   // behind the z pass: nobody waits
             typedef LOp<NZ> L;
 #pragma unroll
             for (int m = 0; m < L::R; ++m)
@@ -289,6 +316,7 @@ __global__ void __maxnreg__(MAXR) k5_happly_yz(HArgs a)
                     Ws[(size_t)(2 * pair) * nxyz + gi] = wu; Ws[(size_t)(2 * pair + 1) * nxyz + gi] = wd;
                 }
         }
+        if (ASYNC) mbar_arrive(barE + buf);                 // this thread is done with unit u
         if (NBUF == 1) { __syncthreads(); if (u + a.G < nunits) issue(u + a.G, 0); }
     }
 }
@@ -328,6 +356,19 @@ __global__ void __maxnreg__(MAXR) k5_happly_xz(HArgs a)
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, g = lane >> 2, t = lane & 3;
     const int nunits = a.ns * UPS;
 
+    // ASYNC: mbarriers F[buf] ("unit landed") and E[buf] ("everyone is done with the unit in buf") instead of a CTA-wide
+    // barrier per unit; see k5_happly_yz.  Off: with one task per warp and unit the prefetch would be issued behind
+    // that task and land too late (measured: 17.6 ms against 14.8 ms per step on config 1).
+    constexpr bool ASYNC = false;
+    __shared__ unsigned long long s_bar[4];
+    unsigned long long *barF = s_bar, *barE = s_bar + 2;
+    if (ASYNC) {
+        if (threadIdx.x == 0) {
+            mbar_init(barF, NWARP * 32); mbar_init(barF + 1, NWARP * 32);
+            mbar_init(barE, NWARP * 32); mbar_init(barE + 1, NWARP * 32);
+        }
+        __syncthreads();
+    }
     auto issue = [&](int u, int buf) {
         const int st = u / UPS, pg = u - st * UPS;
         const size_t go = ((size_t)st * 4 + pg * NCOMP) * nxyz + gb;
@@ -339,7 +380,7 @@ __global__ void __maxnreg__(MAXR) k5_happly_xz(HArgs a)
             cp_async16(dphi + c * PP + x * LD + z, a.X + gi);
             if (WST) cp_async16(dw + c * PP + x * LD + z, a.W + gi);
         }
-        cp_async_commit();
+        if (ASYNC) mbar_arrive_cp_async(barF + buf); else cp_async_commit();
     };
     auto flush_eta = [&](int uprev, int it_prev) {          // thread 0: fixed-order sum of the warps' partials
         const int st = uprev / UPS, pg = uprev - st * UPS;
@@ -351,13 +392,27 @@ __global__ void __maxnreg__(MAXR) k5_happly_xz(HArgs a)
     int u = blockIdx.y, uprev = -1;
     if (u < nunits) issue(u, 0);
     stage_pots();                                           // behind the first prefetch
+    if (ASYNC) __syncthreads();
     int it = 0;
     for (; u < nunits; u += a.G, ++it) {
         const int buf = (NBUF == 2) ? (it & 1) : 0;
-        cp_async_wait<0>();
-        __syncthreads();
-        if (NBUF == 2 && u + a.G < nunits) issue(u + a.G, buf ^ 1);
-        if (threadIdx.x == 0 && uprev >= 0) flush_eta(uprev, it - 1);
+        if (ASYNC) mbar_wait(barF + buf, (it >> 1) & 1);
+        else {
+            cp_async_wait<0>();
+            __syncthreads();
+            if (NBUF == 2 && u + a.G < nunits) issue(u + a.G, buf ^ 1);
+            if (threadIdx.x == 0 && uprev >= 0) flush_eta(uprev, it - 1);
+        }
+        bool mid_done = false;
+        auto mid_unit = [&]() {                             // once per unit and thread, behind the first x pass
+            if (!ASYNC || mid_done) return;
+            mid_done = true;
+            if (it >= 1) {
+                mbar_wait(barE + (buf ^ 1), ((it - 1) >> 1) & 1);       // everyone is done with unit u - G
+                if (threadIdx.x == 0) flush_eta(uprev, it - 1);
+            }
+            if (u + a.G < nunits) issue(u + a.G, buf ^ 1);
+        };
         const int st = u / UPS, pg = u - st * UPS;
         const cplx* phib = phi + buf * NCOMP * PP;
         double eta_loc = 0.0;
@@ -384,6 +439,7 @@ __global__ void __maxnreg__(MAXR) k5_happly_xz(HArgs a)
             cplx ru[NA], rd[NA];
             if (pair) taxis_core5<NX, 0, true>(fu, fd, potx, l0, 1, LD, s_tx, ru, rd);
             else      taxis_core5<NX, 0, false>(fu, fd, potx, l0, 1, LD, s_tx, ru, rd);
+            mid_unit();
 #pragma unroll
             for (int m = 0; m < L::R; ++m)
 #pragma unroll
@@ -401,7 +457,9 @@ __global__ void __maxnreg__(MAXR) k5_happly_xz(HArgs a)
                 }
         }
         for (int o = 16; o > 0; o >>= 1) eta_loc += __shfl_xor_sync(0xffffffffu, eta_loc, o);
+        mid_unit();
         if (lane == 0) s_red[(it & 1) * NWARP + warp] = eta_loc;
+        if (ASYNC) mbar_arrive(barE + buf);
         uprev = u;
         if (NBUF == 1) { __syncthreads(); if (u + a.G < nunits) issue(u + a.G, 0); }
     }

@@ -23,6 +23,32 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int NPENDING>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(NPENDING) : "memory"); }
 
+// ---- shared-memory mbarriers: split arrive / wait, so that a warp signals "done" and runs on instead of stopping at a
+// CTA-wide barrier (the plane kernels let their warps drift apart by up to one task) ----
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, int count)
+{
+    const unsigned s = (unsigned)__cvta_generic_to_shared(bar);
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(s), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long* bar)
+{
+    const unsigned s = (unsigned)__cvta_generic_to_shared(bar);
+    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}" ::"r"(s) : "memory");
+}
+// the executing thread's earlier cp.async copies arrive on the barrier when they have landed (count not incremented:
+// the barrier's expected count includes this arrival)
+__device__ __forceinline__ void mbar_arrive_cp_async(unsigned long long* bar)
+{
+    const unsigned s = (unsigned)__cvta_generic_to_shared(bar);
+    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(s) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity)
+{
+    const unsigned s = (unsigned)__cvta_generic_to_shared(bar);
+    asm volatile("{\n\t.reg .pred p;\n\tWAIT_%=:\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t@p bra DONE_%=;\n\tbra WAIT_%=;\n\tDONE_%=:\n\t}"
+                 ::"r"(s), "r"(parity) : "memory");
+}
+
 // compact potentials of one plane for one axis, in shared memory (doubles, same padded layout as the planes)
 //   B_i = A_i + (sigma x W)_i / 2:  x: b00 = A - hWy, b11 = A + hWy, b01 = (0, -hWz)
 //                                   y: b00 = A + hWx, b11 = A - hWx, b01 = (-hWz, 0)
