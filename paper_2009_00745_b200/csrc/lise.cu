@@ -44,6 +44,10 @@ struct lise_ctx {
     cudaStream_t streamH;                   // highest priority: the DMMA kernels of lise_step run here when overlap is on, so
                                             // that their CTAs are placed first and the update CTAs fill the room left beside them
     cudaEvent_t ev_fork, ev_join;
+    cudaStream_t streamH2;                  // second high-priority stream: the H-apply kernels of odd chunks run here, so that the
+                                            // tail of one chunk's kernels and the head of the next chunk's overlap on the SMs
+    cudaEvent_t ev_h2a, ev_h2b;
+    int twostream;
     cudaStream_t user_stream; int user_stream_valid;   // the caller's stream while lise_step runs on streamH
     cudaEvent_t ev_h[2], ev_u[2];
     int overlap, dgroup;                    // dgroup: chunks per density-kernel launch
@@ -552,8 +556,14 @@ static int abm_step(lise_ctx* c)
     const size_t slen = (size_t)4 * c->L.nxyz;
     TRY(ensure_potentials(c));                      // potentials of y_n
     const bool pipe = c->ks.v5 && c->overlap;
+    // two H-apply streams only while lise_step runs on the internal stream (both are internal, same priority)
+    const bool two = pipe && c->twostream && c->user_stream_valid && c->stream == c->streamH;
+    cudaStream_t const smain = c->stream;
     for (int phase = 1; phase <= 2; ++phase) {
         TRY(zero_partials(c, 0)); TRY(zero_partials(c, 1));
+        if (two) {                                  // the second stream starts behind the potentials of this phase
+            CK(cudaEventRecord(c->ev_h2a, smain)); CK(cudaStreamWaitEvent(c->streamH2, c->ev_h2a, 0));
+        }
         int i = 0;                                  // chunk counter across both species
         // densities of the new state: accumulated over groups of `dgroup` chunks (one launch pair per group), behind
         // the H-apply of the following chunk so that the update of the last chunk of the group overlaps it
@@ -571,11 +581,15 @@ static int abm_step(lise_ctx* c)
                 const size_t off = s0 * slen;
                 const int wb = pipe ? (i & 1) : 0;
                 const cplx* X = (phase == 1 ? S(c, q, RA) : S(c, q, RF)) + off;
-                if (pipe && i >= 2) CK(cudaStreamWaitEvent(c->stream, c->ev_u[wb], 0));   // W[wb], eta[wb] are free again
-                TRY(apply_h_chunk(c, q, X, Wbuf(c, wb), etabuf(c, wb), ns));
+                cudaStream_t sh = (two && (i & 1)) ? c->streamH2 : smain;      // this chunk's H-apply stream
+                if (pipe && i >= 2) CK(cudaStreamWaitEvent(sh, c->ev_u[wb], 0));   // W[wb], eta[wb] are free again
+                c->stream = sh;
+                const int rch = apply_h_chunk(c, q, X, Wbuf(c, wb), etabuf(c, wb), ns);
+                c->stream = smain;
+                TRY(rch);
                 UArgs u = make_uargs(c, q, off, ns, wb);
                 cudaStream_t su = pipe ? c->stream2 : c->stream;
-                if (pipe) { CK(cudaEventRecord(c->ev_h[wb], c->stream)); CK(cudaStreamWaitEvent(c->stream2, c->ev_h[wb], 0)); }
+                if (pipe) { CK(cudaEventRecord(c->ev_h[wb], sh)); CK(cudaStreamWaitEvent(c->stream2, c->ev_h[wb], 0)); }
                 if (phase == 1) TRY(launch_update<1>(c, u, su)); else TRY(launch_update<2>(c, u, su));
                 if (pipe) CK(cudaEventRecord(c->ev_u[wb], c->stream2));
                 if (c->ks.v5) {
@@ -587,6 +601,10 @@ static int abm_step(lise_ctx* c)
                 }
             }
         TRY(flush_dens(i - 1));
+        if (two) {                                  // join the second stream (its last H-apply is ordered before the last updates,
+            CK(cudaEventRecord(c->ev_h2b, c->streamH2));   // which flush_dens waited for, but make the join explicit)
+            CK(cudaStreamWaitEvent(smain, c->ev_h2b, 0));
+        }
         if (phase == 1) TRY(grid_phase(c, 1));     // potentials of the modifier m
     }
     // y_{n+1} sits in B: A <-> B; f history shifts
@@ -773,6 +791,11 @@ static int ctx_init(lise_ctx* c)
         CK(cudaDeviceGetStreamPriorityRange(&lo, &hi));
         CK(cudaStreamCreateWithPriority(&c->stream2, cudaStreamNonBlocking, lo));
         CK(cudaStreamCreateWithPriority(&c->streamH, cudaStreamNonBlocking, hi));
+        CK(cudaStreamCreateWithPriority(&c->streamH2, cudaStreamNonBlocking, hi));
+        CK(cudaEventCreateWithFlags(&c->ev_h2a, cudaEventDisableTiming));
+        CK(cudaEventCreateWithFlags(&c->ev_h2b, cudaEventDisableTiming));
+        c->twostream = 0;                   // measured: no gain on config 1 (60.7 against 60.5 ms per step); kept as an option
+        if (const char* e = getenv("LISE_TWOSTREAM")) c->twostream = atoi(e) ? 1 : 0;
         CK(cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
         CK(cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming));
     }
@@ -863,6 +886,9 @@ extern "C" void lise_destroy(lise_ctx* c)
     cudaStreamSynchronize(c->stream);
     if (c->stream2) { cudaStreamSynchronize(c->stream2); cudaStreamDestroy(c->stream2); }
     if (c->streamH) { cudaStreamSynchronize(c->streamH); cudaStreamDestroy(c->streamH); }
+    if (c->streamH2) { cudaStreamSynchronize(c->streamH2); cudaStreamDestroy(c->streamH2); }
+    if (c->ev_h2a) cudaEventDestroy(c->ev_h2a);
+    if (c->ev_h2b) cudaEventDestroy(c->ev_h2b);
     if (c->ev_fork) cudaEventDestroy(c->ev_fork);
     if (c->ev_join) cudaEventDestroy(c->ev_join);
     for (int i = 0; i < 2; ++i) { if (c->ev_h[i]) cudaEventDestroy(c->ev_h[i]); if (c->ev_u[i]) cudaEventDestroy(c->ev_u[i]); }
