@@ -155,8 +155,9 @@ def run_ours(args):
     S = 64.0 * nxyz
     # capacity rule: 7 resident state arrays + scratch must fit; shrink to a multiple of 256 if not
     free, total = torch.cuda.mem_get_info(dev)
-    per_state = 7 * S
-    cap = int((free - 8 * 2 ** 30) / per_state)
+    # 7 resident arrays + one species' input block and its orthonormalisation workspace while the inputs are generated
+    per_state = 9 * S
+    cap = int((free - 12 * 2 ** 30) / per_state)
     req = nwf
     if nwf[0] + nwf[1] > cap:
         each = max(256, (cap // 2) // 256 * 256)
