@@ -121,6 +121,30 @@ def test_chunk_size_does_not_change_results():
         assert rel(d, res[0][1]) < 1e-13
 
 
+def test_stream_overlap_does_not_change_results():
+    """lise_set_overlap (update kernels on a second stream beside the tensor-core kernels, several chunks in flight,
+    densities per group of chunks) is a scheduling choice: bit-identical wavefunctions, densities and energy."""
+    from paper_2009_00745_b200 import lise
+    cfg = dict(inputs.CONFIGS[1]); cfg["shape"] = (16, 16, 16)
+    nwf = (29, 23)
+    psi = [inputs.make_species(cfg, q, nwf[q], seed=11).cuda() for q in (0, 1)]
+    res = []
+    for overlap in (True, False):
+        g = lise.Lise(*cfg["shape"], cfg["dx"], cfg["dt"], *nwf)
+        g.set_chunk(4)                               # many chunks, ragged tail
+        g.set_overlap(overlap)
+        for q in (0, 1):
+            g.set_wavefunctions(q, psi[q])
+        g.step(6)
+        res.append(([g.get_wavefunctions(q).cpu().numpy() for q in (0, 1)],
+                    [g.densities(q).cpu().numpy() for q in (0, 1)], g.observables()["energy"]))
+        g.close()
+    for q in (0, 1):
+        assert np.array_equal(res[0][0][q], res[1][0][q])
+        assert np.array_equal(res[0][1][q], res[1][1][q])
+    assert res[0][2] == res[1][2]
+
+
 def test_edge_cases_and_errors():
     from paper_2009_00745_b200 import lise
     import ctypes as C
