@@ -263,9 +263,12 @@ static constexpr size_t v5_smem_happly_xz(int ncomp, int nbuf, int nwarp, bool w
     return 8 * ((tabsz<NX>() + 1) / 2 * 2) + 16 * (size_t)(NX * ldpad(NZ)) * ncomp * nbuf * (wst ? 2 : 1) + 8 * (size_t)(NX * ldpad(NZ)) * 4 + 8 * 2 * nwarp;
 }
 template <int NY, int NZ>
-static constexpr size_t v5_smem_dens_yz() { return 8 * ((tabsz<NY>() + tabsz<NZ>() + 1) / 2 * 2) + 16 * (size_t)(4 * NY * ldpad(NZ)); }
+static constexpr size_t v5_smem_dens_yz(int sb) { return 8 * ((tabsz<NY>() + tabsz<NZ>() + 1) / 2 * 2) + 16 * (size_t)(4 * sb * NY * ldpad(NZ)); }
 template <int NX, int NZ>
-static constexpr size_t v5_smem_dens_x() { return 8 * ((tabsz<NX>() + 1) / 2 * 2) + 16 * (size_t)(4 * NX * ldpad(NZ)); }
+static constexpr size_t v5_smem_dens_x(int sb) { return 8 * ((tabsz<NX>() + 1) / 2 * 2) + 16 * (size_t)(4 * sb * NX * ldpad(NZ)); }
+// states per barrier round of a density kernel: up to 4, as many as fit half of the shared memory 
+template <int N1, int NZ>
+static constexpr int v5_dens_sb() { return (16 * (size_t)(4 * 4 * N1 * ldpad(NZ)) <= 180 * 1024) ? 4 : (16 * (size_t)(4 * 2 * N1 * ldpad(NZ)) <= 180 * 1024) ? 2 : 1; }
 static constexpr int imin(int a, int b) { return a < b ? a : b; }
 static constexpr int imax(int a, int b) { return a > b ? a : b; }
 // warps per 2-spinor of an H-apply CTA: one strip task per warp if possible; long lines need more registers per thread
@@ -314,11 +317,12 @@ static KernSet make_v5_set()
     k.h_yz = k5_happly_yz<NY, NZ, CYZ, BYZ, WYZ, VST, RYZ>; k.h_xz = k5_happly_xz<NX, NZ, CXZ, BXZ, WXZ, RXZ, WST>;
     k.cps_h[0] = TWO_YZ ? 2 : 1; k.cps_h[1] = TWO_XZ ? 2 : 1;
     k.u[0] = nullptr; k.u[1] = k5_update<1>; k.u[2] = k5_update<2>; k.u[3] = k5_update<3>;
-    k.d_yz = k5_dens_yz<NY, NZ, WDY>; k.d_x = k5_dens_x<NX, NZ, WDX>;
+    constexpr int SBY = v5_dens_sb<NY, NZ>(), SBX = v5_dens_sb<NX, NZ>();
+    k.d_yz = k5_dens_yz<NY, NZ, WDY, SBY>; k.d_x = k5_dens_x<NX, NZ, WDX, SBX>;
     k.name = "dmma"; k.v5 = 1;
     k.thr_h[0] = 32 * WYZ; k.thr_h[1] = 32 * WXZ; k.thr_u = LISE_UPD_THREADS; k.thr_d = 32 * WDX; k.thr_dyz = 32 * WDY;
     k.smem_h[0] = v5_smem_happly_yz<NY, NZ>(CYZ, BYZ, VST); k.smem_h[1] = v5_smem_happly_xz<NX, NZ>(CXZ, BXZ, WXZ, WST);
-    k.smem_u = 0; k.smem_d = v5_smem_dens_x<NX, NZ>(); k.smem_dyz = v5_smem_dens_yz<NY, NZ>();
+    k.smem_u = 0; k.smem_d = v5_smem_dens_x<NX, NZ>(SBX); k.smem_dyz = v5_smem_dens_yz<NY, NZ>(SBY);
     k.ups_xz = 4 / CXZ;
     return k;
 }

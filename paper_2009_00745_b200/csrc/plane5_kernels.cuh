@@ -654,9 +654,9 @@ __device__ __forceinline__ void dens_task_flush5(double* __restrict__ part, int 
 // densities of the states in Z on yz-planes: pointwise n, s, kappa (Eq. 3a, 3d, 3b) and the y/z-line parts of
 // t, j, J.  grid (nx, G), NWARP warps; v_up, v_dn planes prefetched by cp.async (two buffers), one barrier per state.
 // Every accumulator lives in registers for the whole launch (fixed thread <-> point maps) and is added to part[g]
-// at the end, map by map (deterministic).   shared: tables | v[2][2][PP]
+// at the end, map by map (deterministic).   shared: tables | v[2][SB][2][PP]
 // ------------------------------------------------------------------------------------------------
-template <int NY, int NZ, int NWARP>
+template <int NY, int NZ, int NWARP, int SB>
 __global__ void __launch_bounds__(NWARP * 32, 1) k5_dens_yz(DArgs a)
 {
     extern __shared__ double2 smem[];
@@ -683,24 +683,32 @@ __global__ void __launch_bounds__(NWARP * 32, 1) k5_dens_yz(DArgs a)
         for (int r = 0; r < NAM; ++r) acct[i][r][0] = acct[i][r][1] = acct[i][r][2] = 0.0;
     const int warp = threadIdx.x >> 5;
 
-    auto issue = [&](int st, int buf) {
-        const cplx* Zs = a.Z + ((size_t)st * 4 + 2) * nxyz + gbase;
-        cplx* dst = vpl + buf * 2 * PP;
-        for (int i = threadIdx.x; i < 2 * NPTS; i += blockDim.x) {
-            const int c = i / NPTS, p = i - c * NPTS, y = p / NZ, z = p - y * NZ;
-            cp_async16(dst + c * PP + y * LD + z, Zs + (size_t)c * nxyz + p);
+    // a batch = SB states of this CTA's group (one barrier and one prefetch per batch, not per state)
+    auto issue = [&](int st0, int buf) {
+        for (int j = 0; j < SB; ++j) {
+            const int st = st0 + j * a.G;
+            if (st >= a.ns) break;
+            const cplx* Zs = a.Z + ((size_t)st * 4 + 2) * nxyz + gbase;
+            cplx* dst = vpl + (buf * SB + j) * 2 * PP;
+            for (int i = threadIdx.x; i < 2 * NPTS; i += blockDim.x) {
+                const int c = i / NPTS, p = i - c * NPTS, y = p / NZ, z = p - y * NZ;
+                cp_async16(dst + c * PP + y * LD + z, Zs + (size_t)c * nxyz + p);
+            }
         }
         cp_async_commit();
     };
 
-    int st = blockIdx.y;
-    if (st < a.ns) issue(st, 0);
-    for (int it = 0; st < a.ns; st += a.G, ++it) {
+    int st0 = blockIdx.y;
+    if (st0 < a.ns) issue(st0, 0);
+    for (int it = 0; st0 < a.ns; st0 += SB * a.G, ++it) {
         const int buf = it & 1;
         cp_async_wait<0>();
         __syncthreads();
-        if (st + a.G < a.ns) issue(st + a.G, buf ^ 1);
-        const cplx *vu_p = vpl + buf * 2 * PP, *vd_p = vu_p + PP;
+        if (st0 + SB * a.G < a.ns) issue(st0 + SB * a.G, buf ^ 1);
+        for (int j = 0; j < SB; ++j) {
+        const int st = st0 + j * a.G;
+        if (st >= a.ns) break;
+        const cplx *vu_p = vpl + (buf * SB + j) * 2 * PP, *vd_p = vu_p + PP;
         // the up component of u for kappa: issued before the DMMA work, consumed after it
         cplx uu[NIT];
 #pragma unroll
@@ -739,6 +747,7 @@ __global__ void __launch_bounds__(NWARP * 32, 1) k5_dens_yz(DArgs a)
             accp[i][4] += vd.x * nu0.x + vd.y * nu0.y;      // conj(v_dn) u_up
             accp[i][5] += vd.x * nu0.y - vd.y * nu0.x;
         }
+        }
     }
     double* part = a.part + (size_t)blockIdx.y * LISE_NACC * nxyz;
     const int prow[6] = {ACC_N, ACC_S + 0, ACC_S + 1, ACC_S + 2, ACC_K + 0, ACC_K + 1};
@@ -771,7 +780,7 @@ __global__ void __launch_bounds__(NWARP * 32, 1) k5_dens_yz(DArgs a)
 }
 
 // x-axis density pass of the states in Z.   grid (ny, G), NWARP warps.  shared: table | v[2][2][PP]
-template <int NX, int NZ, int NWARP>
+template <int NX, int NZ, int NWARP, int SB>
 __global__ void __launch_bounds__(NWARP * 32, 1) k5_dens_x(DArgs a)
 {
     extern __shared__ double2 smem[];
@@ -790,24 +799,30 @@ __global__ void __launch_bounds__(NWARP * 32, 1) k5_dens_x(DArgs a)
         for (int r = 0; r < NA; ++r) acc[i][r][0] = acc[i][r][1] = acc[i][r][2] = 0.0;
     const int warp = threadIdx.x >> 5;
 
-    auto issue = [&](int st, int buf) {
-        const cplx* Zs = a.Z + ((size_t)st * 4 + 2) * nxyz + gb;
-        cplx* dst = vpl + buf * 2 * PP;
-        for (int i = threadIdx.x; i < 2 * NPTS; i += blockDim.x) {
-            const int c = i / NPTS, p = i - c * NPTS, x = p / NZ, z = p - x * NZ;
-            cp_async16(dst + c * PP + x * LD + z, Zs + (size_t)c * nxyz + (size_t)x * gs + z);
+    auto issue = [&](int st0, int buf) {
+        for (int j = 0; j < SB; ++j) {
+            const int st = st0 + j * a.G;
+            if (st >= a.ns) break;
+            const cplx* Zs = a.Z + ((size_t)st * 4 + 2) * nxyz + gb;
+            cplx* dst = vpl + (buf * SB + j) * 2 * PP;
+            for (int i = threadIdx.x; i < 2 * NPTS; i += blockDim.x) {
+                const int c = i / NPTS, p = i - c * NPTS, x = p / NZ, z = p - x * NZ;
+                cp_async16(dst + c * PP + x * LD + z, Zs + (size_t)c * nxyz + (size_t)x * gs + z);
+            }
         }
         cp_async_commit();
     };
 
-    int st = blockIdx.y;
-    if (st < a.ns) issue(st, 0);
-    for (int it = 0; st < a.ns; st += a.G, ++it) {
+    int st0 = blockIdx.y;
+    if (st0 < a.ns) issue(st0, 0);
+    for (int it = 0; st0 < a.ns; st0 += SB * a.G, ++it) {
         const int buf = it & 1;
         cp_async_wait<0>();
         __syncthreads();
-        if (st + a.G < a.ns) issue(st + a.G, buf ^ 1);
-        const cplx *vu_p = vpl + buf * 2 * PP, *vd_p = vu_p + PP;
+        if (st0 + SB * a.G < a.ns) issue(st0 + SB * a.G, buf ^ 1);
+        for (int j = 0; j < SB; ++j) {
+        if (st0 + j * a.G >= a.ns) break;
+        const cplx *vu_p = vpl + (buf * SB + j) * 2 * PP, *vd_p = vu_p + PP;
 #pragma unroll
         for (int i = 0; i < TPW; ++i) {
             const int task = warp + i * NWARP;
@@ -816,6 +831,7 @@ __global__ void __launch_bounds__(NWARP * 32, 1) k5_dens_x(DArgs a)
                 if (task & 1) dens_axis_task5<NX, 0, 1>(vu_p, vd_p, acc[i], l0, 1, LD, s_tx);
                 else          dens_axis_task5<NX, 0, 0>(vu_p, vd_p, acc[i], l0, 1, LD, s_tx);
             }
+        }
         }
     }
     double* part = a.part + (size_t)blockIdx.y * LISE_NACC * nxyz;
