@@ -36,6 +36,22 @@ def read_peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
+def measured_traffic(cls, workload, states_per_launch):
+    """DRAM bytes per launch of kernel class `cls` from the committed ncu capture (profiles/r1_v5_traffic.md: bytes per
+    state on the config-1 lattice), or None for other workloads / when the file is absent."""
+    if not workload.startswith("config1"):
+        return None
+    path = os.path.join(ROOT, "profiles", "r1_v5_traffic.md")
+    try:
+        for line in open(path):
+            cells = [c.strip() for c in line.strip().strip("|").split("|")]
+            if len(cells) == 5 and cells[0] == cls:
+                return float(cells[4]) * states_per_launch
+    except OSError:
+        pass
+    return None
+
+
 class ClockSampler:
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
@@ -279,7 +295,7 @@ def run_ours(args):
     roof["kernel"] = top
     roof["avg_launch_ms"] = avg_s * 1e3
     roof["share_of_step"] = top_ms / tot_ms if tot_ms > 0 else None
-    roof["traffic"] = None
+    roof["traffic"] = measured_traffic(top, cfg["name"], states_per_launch)
     roof["classes_ms_per_step"] = {k: v[0] / psteps for k, v in prof.items()}
     roof["classes_note"] = "per-class device time with the update/H-apply stream overlap off; the timed region runs with it on"
     step_bytes = 15.0 * S                                              # B_min = 960 Nxyz per qpwf-update
