@@ -121,6 +121,58 @@ def test_chunk_size_does_not_change_results():
         assert rel(d, res[0][1]) < 1e-13
 
 
+def test_full_size_config1_in_the_bench_launch_configuration():
+    """BASELINE.json configs[1] at its full size (24^3, 4096 + 4096 states, the launch configuration bench.py times:
+    default chunk, stream overlap on).  The oracle cannot step 8192 states, so: (i) the densities of ALL states against
+    the oracle's densities_of, streamed in blocks (densities are sums over states); (ii) the potentials against the
+    oracle's potentials_from those densities; (iii) H psi on a seeded sample of 64 states per species against the
+    oracle's apply_h_with; (iv) after 3 starter + 2 ABM steps the invariants that hold at any size: norm and
+    orthonormality defects, particle numbers and energy drift at the level SURVEY 8(c) states for incomplete sets."""
+    from paper_2009_00745_b200 import lise
+    free, _ = torch.cuda.mem_get_info()
+    cfg = dict(inputs.CONFIGS[1])
+    nwf = tuple(cfg["nwf"])
+    S = 64.0 * np.prod(cfg["shape"])
+    if free < 9.5 * S * sum(nwf) + 8 * 2 ** 30:
+        pytest.skip("not enough free device memory for the full-size workload")
+    shape = tuple(cfg["shape"])
+    seed = inputs.SEED0 + 1
+    g = lise.Lise(*shape, cfg["dx"], cfg["dt"], *nwf)
+    oc = ref.RefContext(*shape, cfg["dx"], cfg["dt"], 1, 1)          # used for its stateless entry points only
+    rng = np.random.default_rng(2009)
+    dens_ref, sample = [], []
+    for q in (0, 1):
+        psi = inputs.make_block(cfg, q, nwf[q], 0, nwf[q], seed, "cuda")
+        g.set_wavefunctions(q, psi)
+        acc = np.zeros((14,) + shape)
+        for f in range(0, nwf[q], 512):
+            acc += oc.densities_of(psi[f:f + 512].cpu().numpy()).reshape(acc.shape)
+        dens_ref.append(acc)
+        idx = np.sort(rng.choice(nwf[q], size=64, replace=False))
+        sample.append(psi[torch.as_tensor(idx, device="cuda")].contiguous())
+        del psi
+    # rows of Table 2 that are grid derivatives of the accumulated fields (tau, div J, curl j) are not additive in the
+    # way densities_of reports them only if it applied them per block: they are linear, so the block sum is exact
+    for q in (0, 1):
+        d_gpu = g.densities(q).cpu().numpy()
+        assert field_rel(d_gpu, dens_ref[q]) < TOL_DENS, ("densities", q)
+    pots = oc.potentials_from(dens_ref[0], dens_ref[1])
+    for q in (0, 1):
+        p_gpu = g.potentials(q).cpu().numpy()
+        assert field_rel(p_gpu, np.asarray(pots[q]).reshape(p_gpu.shape)) < 1e-10, ("potentials", q)
+        h_ref = oc.apply_h_with(np.asarray(pots[q]), sample[q].cpu().numpy()).reshape(sample[q].shape)
+        h_gpu = g.apply_h(q, sample[q]).cpu().numpy()
+        assert rel(h_gpu, h_ref) < 1e-12, ("H psi", q)
+    o0 = g.observables()
+    g.step(5)
+    o1 = g.observables()
+    assert o1["norm_defect"] < 1e-10 and o1["ortho_defect"] < 1e-10
+    assert abs(o1["energy"] - o0["energy"]) < 1e-4 * abs(o0["energy"])
+    for k in ("n_neutron", "n_proton"):
+        assert abs(o1[k] - o0[k]) < 1e-4 * o0[k]
+    g.close(); oc.close()
+
+
 def test_stream_overlap_does_not_change_results():
     """lise_set_overlap (update kernels on a second stream beside the tensor-core kernels, several chunks in flight,
     densities per group of chunks) is a scheduling choice: bit-identical wavefunctions, densities and energy."""
