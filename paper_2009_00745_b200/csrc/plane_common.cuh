@@ -9,11 +9,6 @@
 
 __host__ __device__ constexpr int ldpad(int n) { return n + ((4 - n % 8) + 8) % 8; }
 
-__device__ __forceinline__ void dmma4(double (&d)[2], double a, double b)
-{
-    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
-        : "+d"(d[0]), "+d"(d[1]) : "d"(a), "d"(b));
-}
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc)
 {
     const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
@@ -59,14 +54,6 @@ struct AxisPot4 {
     const double* w1;     // x: hWy   y: hWx   z: hWy
     const double* w2;     // x: hWz   y: hWz   z: hWx
 };
-
-template <int AXIS>
-__device__ __forceinline__ void make_B4(double A, double w1, double w2, double& b00, double& b11, double& br, double& bi)
-{
-    if (AXIS == 0)      { b00 = A - w1; b11 = A + w1; br = 0.0; bi = -w2; }
-    else if (AXIS == 1) { b00 = A + w1; b11 = A - w1; br = -w2; bi = 0.0; }
-    else                { b00 = A;      b11 = A;      br = w1;  bi = w2; }
-}
 
 // the part (re if !im, im if im) of g = -i B phi this lane feeds to the tensor core
 template <int AXIS>

@@ -8,7 +8,8 @@
 // and every T_i acts on independent lattice lines along axis i.  A CTA therefore works on one
 // lattice PLANE staged in shared memory: yz-planes (contiguous in memory) carry the y and z lines,
 // xz-planes carry the x lines.  D_i, D2_i are applied to a line as circulant sums with the
-// closed-form DVR coefficients of PAPER.md Eq. 48 (v1 line operator; see fft_lines.cuh for the FFT one).
+// closed-form DVR coefficients of PAPER.md Eq. 48 (generic DFMA line operator: any even lattice; the lattices the
+// library is instantiated for run the tensor-core kernels of plane5_kernels.cuh instead).
 #pragma once
 #include "common.cuh"
 
@@ -71,136 +72,9 @@ __device__ __forceinline__ void line_apply(const cplx* __restrict__ srcA, const 
     }
 }
 
-// ------------------------------------------------------------------------------------------------
-// line operator on the fp64 tensor-core path: the circulant sums written as 8x8x4 DMMA tiles
-// (mma.sync.aligned.m8n8k4 f64; SASS DMMA.8x8x4).  PAPER.md Eq. 45-48 state the lattice derivative as
-// the dense DVR matrix (d/dx)_{nm}; applied to the lines of a plane it is a real (N x N) x (N x 2*lines)
-// contraction, re and im parts as separate columns.  B200 issues 64 fp64 FMA/clk/SM through either DFMA
-// or DMMA (measured: 33.1 vs 37.1 TFLOP/s, same pipe); DMMA needs one issue slot and no shared-memory
-// operand per 256 FMAs, where the DFMA loop above needs one LDS per 4.
-//
-// A warp task = one component x one strip of 8 lines x all N outputs.  Thread (g = lane/4, t = lane%4).
-//   column lines (ROW = false; points along n1, stride ld): out[n][z] = sum_m c[n-m] x[m][z]
-//       A = circulant tile  (thread: c[(8r+g) - (4k+t)]),  B = x tile (thread: x[4k+t][z0+g])
-//   row lines    (ROW = true;  points along n2, stride 1):  out[l][n] = sum_m x[l][m] c[n-m]
-//       A = x tile (thread: x[l0+g][4k+t]),  B = circulant tile (thread: c[(8r+g) - (4k+t)], same registers)
-//   accumulator: rows g, columns 2t, 2t+1.
-// N % 4 == 0; output rows are padded to a multiple of 8 (padding rows wrap around mod N and are not stored).
-//   MODE 0: dstA = D src, dstB = D2 src.      MODE 1: dstA += D srcA + D2 srcB.
-// ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double b)
-{
-    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
-                 : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
-}
-
-template <int N, bool ROW, int MODE>
-__device__ __forceinline__ void mma_line_apply(const cplx* __restrict__ srcA, const cplx* __restrict__ srcB, int sstride,
-                                               cplx* __restrict__ dstA, cplx* __restrict__ dstB, int dstride,
-                                               int ncomp, int nlines, int ld, const double2* __restrict__ ct)
-{
-    constexpr int NK = N / 4;                 // k steps
-    constexpr int NT = (N + 7) / 8;           // output row tiles
-    constexpr int RT = (NT > 4) ? 4 : NT;     // row tiles per pass (bounds the accumulator registers)
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
-    const int g = lane >> 2, t = lane & 3;
-    // circulant fragments: cf[j] = c[(4j + g - t) mod N]
-    double cf1[NK], cf2[NK];
-#pragma unroll
-    for (int j = 0; j < NK; ++j) {
-        int d = 4 * j + g - t;
-        d = (d + N) % N;
-        const double2 c = ct[N + d];
-        cf1[j] = c.x; cf2[j] = c.y;
-    }
-    const int nstrips = (nlines + 7) >> 3;
-    const int ntask = ncomp * nstrips;
-    for (int task = warp; task < ntask; task += nwarps) {
-        const int c = task / nstrips, l0 = (task - c * nstrips) << 3;
-        const cplx* xa = srcA + c * sstride;
-        const cplx* xb = (MODE == 1) ? (srcB + c * sstride) : xa;
-        // load offset of this thread's operand element at k step 0, and its increment per k step
-        int lofs, linc;
-        if (ROW) { int l = l0 + g; if (l >= nlines) l = nlines - 1; lofs = l * ld + t; linc = 4; }
-        else     { int z = l0 + g; if (z >= nlines) z = nlines - 1; lofs = t * ld + z; linc = 4 * ld; }
-#pragma unroll
-        for (int r0 = 0; r0 < NT; r0 += RT) {
-            double p_re[RT][2], p_im[RT][2], q_re[RT][2], q_im[RT][2];
-#pragma unroll
-            for (int r = 0; r < RT; ++r) {
-                p_re[r][0] = p_re[r][1] = p_im[r][0] = p_im[r][1] = 0.0;
-                q_re[r][0] = q_re[r][1] = q_im[r][0] = q_im[r][1] = 0.0;
-            }
-#pragma unroll
-            for (int k = 0; k < NK; ++k) {
-                const cplx x = xa[lofs + k * linc];
-                cplx y = x;
-                if (MODE == 1) y = xb[lofs + k * linc];
-#pragma unroll
-                for (int r = 0; r < RT; ++r) {
-                    if (r0 + r >= NT) continue;
-                    constexpr int dummy = 0; (void)dummy;
-                    const int j = (((2 * (r0 + r) - k) % NK) + NK) % NK;
-                    if (ROW) {
-                        if (MODE == 0) {
-                            dmma884(p_re[r][0], p_re[r][1], x.x, cf1[j]); dmma884(p_im[r][0], p_im[r][1], x.y, cf1[j]);
-                            dmma884(q_re[r][0], q_re[r][1], x.x, cf2[j]); dmma884(q_im[r][0], q_im[r][1], x.y, cf2[j]);
-                        } else {
-                            dmma884(p_re[r][0], p_re[r][1], x.x, cf1[j]); dmma884(p_im[r][0], p_im[r][1], x.y, cf1[j]);
-                            dmma884(p_re[r][0], p_re[r][1], y.x, cf2[j]); dmma884(p_im[r][0], p_im[r][1], y.y, cf2[j]);
-                        }
-                    } else {
-                        if (MODE == 0) {
-                            dmma884(p_re[r][0], p_re[r][1], cf1[j], x.x); dmma884(p_im[r][0], p_im[r][1], cf1[j], x.y);
-                            dmma884(q_re[r][0], q_re[r][1], cf2[j], x.x); dmma884(q_im[r][0], q_im[r][1], cf2[j], x.y);
-                        } else {
-                            dmma884(p_re[r][0], p_re[r][1], cf1[j], x.x); dmma884(p_im[r][0], p_im[r][1], cf1[j], x.y);
-                            dmma884(p_re[r][0], p_re[r][1], cf2[j], y.x); dmma884(p_im[r][0], p_im[r][1], cf2[j], y.y);
-                        }
-                    }
-                }
-            }
-            // store: accumulator rows g, columns 2t, 2t+1
-            cplx* da = dstA + c * dstride;
-            cplx* db = (MODE == 0) ? (dstB + c * dstride) : da;
-#pragma unroll
-            for (int r = 0; r < RT; ++r) {
-                if (r0 + r >= NT) continue;
-                if (ROW) {
-                    const int l = l0 + g, n = 8 * (r0 + r) + 2 * t;
-                    if (l < nlines && n < N) {            // N even: n + 1 < N as well
-                        const int o = l * ld + n;
-                        if (MODE == 0) {
-                            da[o] = cmk(p_re[r][0], p_im[r][0]); da[o + 1] = cmk(p_re[r][1], p_im[r][1]);
-                            db[o] = cmk(q_re[r][0], q_im[r][0]); db[o + 1] = cmk(q_re[r][1], q_im[r][1]);
-                        } else {
-                            const cplx o0 = da[o], o1 = da[o + 1];
-                            da[o] = cmk(o0.x + p_re[r][0], o0.y + p_im[r][0]);
-                            da[o + 1] = cmk(o1.x + p_re[r][1], o1.y + p_im[r][1]);
-                        }
-                    }
-                } else {
-                    const int n = 8 * (r0 + r) + g, z = l0 + 2 * t;
-                    if (n < N && z < nlines) {            // nlines even: z + 1 < nlines as well
-                        const int o = n * ld + z;
-                        if (MODE == 0) {
-                            da[o] = cmk(p_re[r][0], p_im[r][0]); da[o + 1] = cmk(p_re[r][1], p_im[r][1]);
-                            db[o] = cmk(q_re[r][0], q_im[r][0]); db[o + 1] = cmk(q_re[r][1], q_im[r][1]);
-                        } else {
-                            const cplx o0 = da[o], o1 = da[o + 1];
-                            da[o] = cmk(o0.x + p_re[r][0], o0.y + p_im[r][0]);
-                            da[o + 1] = cmk(o1.x + p_re[r][1], o1.y + p_im[r][1]);
-                        }
-                    }
-                }
-            }
-        }
-    }
-}
-
 // line-operator policies: the kernels below call LO::apply<MODE>(col_lines?, ...)
 //   DenseLines<R>   : DFMA circulant sums, any even N (generic path)
-//   MmaLines<NC,NR> : DMMA tiles, NC = column-line length (n1), NR = row-line length (n2; 0 = unused)
+//   (the fp64 tensor-core line operator lives in split_lineop.cuh / plane5_kernels.cuh and is not a policy of these kernels)
 template <int R>
 struct DenseLines {
     static constexpr int MAXT = 512;
@@ -213,19 +87,6 @@ struct DenseLines {
         else     line_apply<R, MODE>(srcA, srcB, sstride, dstA, dstB, dstride, ncomp, n1, n2, ld, 1, ct);
     }
 };
-template <int NC, int NR>
-struct MmaLines {
-    static constexpr int MAXT = 256;
-    template <int MODE>
-    static __device__ __forceinline__ void apply(bool col, const cplx* srcA, const cplx* srcB, int sstride,
-                                                 cplx* dstA, cplx* dstB, int dstride, int ncomp,
-                                                 int n1, int n2, int ld, const double2* ct)
-    {
-        if (col) mma_line_apply<NC, false, MODE>(srcA, srcB, sstride, dstA, dstB, dstride, ncomp, n2, ld, ct);
-        else if (NR > 0) mma_line_apply<(NR > 0 ? NR : 8), true, MODE>(srcA, srcB, sstride, dstA, dstB, dstride, ncomp, n1, ld, ct);
-    }
-};
-
 // B_i = A_i + (1/2)(sigma x W)_i as (B00, B11, B01); B10 = conj(B01).   (from Eqs. 12, 56)
 __device__ __forceinline__ void make_B(int axis, double A, double Wx, double Wy, double Wz,
                                        double& b00, double& b11, cplx& b01)
