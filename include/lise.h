@@ -9,7 +9,8 @@
  * every garbled or ambiguous passage is listed in DESIGN.md (ledger B1..B27).
  *
  * Conventions
- *   species     0 = neutrons, 1 = protons; nwf_p = 0 means neutrons only (Coulomb then off).
+ *   species     0 = neutrons, 1 = protons; nwf_p = 0 means this context holds no proton states: Coulomb then defaults
+ *               to off (a state-sharded rank without protons switches it on with lise_set_params, see below).
  *   lattice     nx, ny, nz even; lattice constant dx = dy = dz (Eq. 43); volume element dV = dx^3.
  *   wavefunction block ("psi"): [state][component: u_up, u_dn, v_up, v_dn][ix][iy][iz], iz fastest,
  *               interleaved (re, im) doubles (Eq. 1; the order inside xyz is this library's choice).
@@ -48,7 +49,8 @@ typedef struct {
     double hbar2_2m, e2, hbarc;                         /* 20.73553 MeV fm^2, 1.439964 MeV fm, 197.3269804 MeV fm */
     double t0, t1, t2, t3, x0, x1, x2, x3, gamma, W0;   /* Skyrme parameters -> couplings of Eq. 9               */
     double g0_n, g0_p;                                  /* bare pairing couplings, MeV fm^3 (0 = pairing off)    */
-    int coulomb;                                        /* 1: Coulomb direct (Eqs. 58-62) + Slater exchange (Eq. 6) for protons */
+    int coulomb;                                        /* 1: Coulomb direct (Eqs. 58-62) + Slater exchange (Eq. 6) for protons; the flag
+                                                         * alone decides (it must be the same on every rank of a state-sharded run) */
     int pairing_rearrangement;                          /* 1: include d E_pair / d n in U (reading B8) */
     int remove_phase;                                   /* 1: subtract eta_k = <psi_k|H|psi_k> (Eqs. 80-81)      */
 } lise_params;
@@ -79,11 +81,15 @@ int lise_set_stream(lise_ctx *ctx, void *cuda_stream);       /* cudaStream_t own
 int lise_set_dt(lise_ctx *ctx, double dt);
 /* Number of states processed per kernel launch (L2-resident batching of intermediates); <= 0 restores the default. */
 int lise_set_chunk(lise_ctx *ctx, int nstates);
-/* Tensor-core kernels only: enable (default, or LISE_OVERLAP=0/1 in the environment) or disable running the
+/* Tensor-core kernels only: enable (default) or disable running the
  * HBM-bound ABM update kernels on an internal second stream concurrently with the DMMA-bound kernels of the
  * neighbouring chunks.  Results are bit-identical either way.  All work is ordered back into the context's
  * stream before lise_step returns. */
 int lise_set_overlap(lise_ctx *ctx, int enable);
+/* Tensor-core kernels only: the densities of the new states are accumulated once per group of `nchunks` chunks
+ * (default 8; <= 0 restores it): one density launch pair per group instead of one per chunk.  A scheduling choice;
+ * results differ only by the summation order of the partial densities (round-off). */
+int lise_set_density_group(lise_ctx *ctx, int nchunks);
 
 /* Copies nwf_q states in (device pointer, layout above), accumulates their densities and resets the
  * multistep history, step counter and time. */
@@ -150,14 +156,8 @@ int lise_profile_read(lise_ctx *ctx, double *ms, long *counts);
  * (HOST pointer).  sm_mhz_host is reserved (set to 0).  Synchronises. */
 int lise_measure_fp64_peak(void *stream, double seconds, double *tflops_host, double *sm_mhz_host);
 
-/* Microbenchmark behind DESIGN.md's fp64-pipe model: every warp of a 1-CTA-per-SM grid with `warps` warps loops over
- * a bundle of independent m8n8k4 DMMAs and DFMAs (variant 0: 8 DMMA, 1: 16 DFMA, 2: 8 + 8, 3: 8 + 16, 4: 8 + 32,
- * 5: 16 DMMA); writes the SM clocks one bundle iteration takes (wall time x nominal SM clock / iterations) to
- * *clocks_per_iter_host (HOST).  Synchronises; uses the default stream. */
-int lise_measure_fp64_mix(int variant, int warps, double *clocks_per_iter_host);
-
 /* Which line operator the per-state kernels of this context use: "dmma" (fp64 tensor-core tiles, for the
- * lattice shapes the library was instantiated for; LISE_LINE_OP=dense in the environment disables it)
+ * lattice shapes the library was instantiated for)
  * or "dense" (generic DFMA circulant sums, any even lattice).  Both apply the same operator (Eq. 48). */
 const char *lise_line_operator(const lise_ctx *ctx);
 

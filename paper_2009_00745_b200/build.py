@@ -1,4 +1,6 @@
 """Builds liblise.so (the C-ABI CUDA library) in-tree with nvcc for sm_100a."""
+import fcntl
+import glob
 import os
 import subprocess
 
@@ -6,24 +8,39 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "liblise.so")
 SOURCES = ["lise.cu"]
-HEADERS = ["common.cuh", "state_kernels.cuh", "grid_kernels.cuh", "plane_common.cuh", "split_lineop.cuh", "plane5_kernels.cuh", "peak_kernels.cuh", os.path.join("..", "..", "include", "lise.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared"]
+
+
+def _deps():
+    return (glob.glob(os.path.join(CSRC, "*.cu")) + glob.glob(os.path.join(CSRC, "*.cuh"))
+            + glob.glob(os.path.join(CSRC, "*.py")) + [os.path.join(HERE, "..", "include", "lise.h")])
 
 
 def needs_build():
     if not os.path.exists(SO):
         return True
     t = os.path.getmtime(SO)
-    return any(os.path.getmtime(os.path.join(CSRC, f)) > t for f in SOURCES + HEADERS)
+    return any(os.path.getmtime(f) > t for f in _deps())
 
 
 def build(force=False, verbose=False):
+    """Compile under a file lock (several ranks may call this at once): nvcc writes a temporary file that is
+    renamed over liblise.so, so no process can dlopen a partly written library."""
     if not force and not needs_build():
         return SO
-    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", SO] + SOURCES
-    subprocess.run(cmd, check=True, cwd=CSRC)
+    with open(os.path.join(HERE, ".build.lock"), "w") as lock:
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        try:
+            if not force and not needs_build():      # another process built it while we waited
+                return SO
+            nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+            tmp = SO + f".tmp{os.getpid()}"
+            cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SOURCES
+            subprocess.run(cmd, check=True, cwd=CSRC)
+            os.replace(tmp, SO)
+        finally:
+            fcntl.flock(lock, fcntl.LOCK_UN)
     return SO
 
 

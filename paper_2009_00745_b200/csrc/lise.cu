@@ -44,10 +44,6 @@ struct lise_ctx {
     cudaStream_t streamH;                   // highest priority: the DMMA kernels of lise_step run here when overlap is on, so
                                             // that their CTAs are placed first and the update CTAs fill the room left beside them
     cudaEvent_t ev_fork, ev_join;
-    cudaStream_t streamH2;                  // second high-priority stream: the H-apply kernels of odd chunks run here, so that the
-                                            // tail of one chunk's kernels and the head of the next chunk's overlap on the SMs
-    cudaEvent_t ev_h2a, ev_h2b;
-    int twostream;
     cudaStream_t user_stream; int user_stream_valid;   // the caller's stream while lise_step runs on streamH
     cudaEvent_t ev_h[2], ev_u[2];
     int overlap, dgroup;                    // dgroup: chunks per density-kernel launch
@@ -113,6 +109,15 @@ static const char* g_noctx = "no context";
 #define CKL()                                                                                      \
     do { c->launches++; CK(cudaGetLastError()); } while (0)
 #define TRY(expr) do { int rc_ = (expr); if (rc_ != LISE_OK) return rc_; } while (0)
+
+// nothing may throw across the C ABI: host allocations (std::vector, new) inside an entry point run under this guard
+template <class F>
+static int guarded(F&& f)
+{
+    try { return f(); }
+    catch (const std::bad_alloc&) { return LISE_ENOMEM; }
+    catch (...) { return LISE_ECUDA; }
+}
 
 static int dmalloc(lise_ctx* c, void** p, size_t bytes)
 {
@@ -222,7 +227,7 @@ static void set_physconst(lise_ctx* c)
     k.Ct[1] = -(p.t1 / 8.0) * (0.5 + p.x1) + (p.t2 / 8.0) * (0.5 + p.x2);
     k.CJ[0] = -3.0 * p.W0 / 4.0;                      k.CJ[1] = -p.W0 / 4.0;
     k.g0[0] = p.g0_n; k.g0[1] = p.g0_p;
-    k.coulomb = p.coulomb && c->nwf[1] > 0; k.rearr = p.pairing_rearrangement;
+    k.coulomb = p.coulomb; k.rearr = p.pairing_rearrangement;
 }
 
 extern "C" int lise_default_params(lise_params* p)
@@ -289,14 +294,11 @@ static constexpr int v5_warps(int tasks, int cap)
     for (int w = cap; w >= cap / 2; --w) if (tasks % w == 0) return w;
     return cap;
 }
-// VAR 0: one plane-owner CTA per SM, whole states if shared memory allows.
-// VAR 1: two CTAs per SM working on 2-spinors (their barrier and epilogue phases interleave) where two fit.
-static constexpr size_t SMEM_HALF = (228 * 1024) / 2 - 1024;
-template <int NX, int NY, int NZ, int VAR>
+// one plane-owner CTA per SM, whole states per unit if shared memory allows
+template <int NX, int NY, int NZ>
 static KernSet make_v5_set()
 {
-    constexpr bool TWO_YZ = VAR == 1 && v5_smem_happly_yz<NY, NZ>(2, 2, false) <= SMEM_HALF && imax(NY, NZ) / 4 <= 8;
-    constexpr bool TWO_XZ = VAR == 1 && v5_smem_happly_xz<NX, NZ>(2, 2, 8) <= SMEM_HALF && NZ / 4 <= 8;
+    constexpr bool TWO_YZ = false, TWO_XZ = false;
     // yz: prefer whole states with prefetch, then 2-spinors with prefetch, then 2-spinors without
     constexpr int CYZ = TWO_YZ ? 2 : (v5_smem_happly_yz<NY, NZ>(4, 2, false) <= SMEM_LIMIT) ? 4 : 2;
     constexpr int BYZ = (v5_smem_happly_yz<NY, NZ>(CYZ, 2, false) <= SMEM_LIMIT) ? 2 : 1;
@@ -332,12 +334,10 @@ static KernSet make_v5_set()
 #define LISE_MMA_SHAPES(X) \
     X(8, 8, 8) X(12, 12, 12) X(16, 16, 16) X(20, 20, 20) X(24, 24, 24) X(32, 32, 32) X(40, 40, 40) \
     X(24, 24, 48) X(24, 24, 64) X(12, 8, 16) X(16, 12, 8)
-static bool pick_kernels(int nx, int ny, int nz, int R, bool want_mma, KernSet* out)
+static bool pick_kernels(int nx, int ny, int nz, int R, KernSet* out)
 {
-    if (want_mma) {
-        // (VAR 1 of make_v5_set -- two CTAs per SM on 2-spinor units -- is kept as a template option but not instantiated:
-        // measured slower on config 1)
-#define X(a, b, c_) if (nx == a && ny == b && nz == c_) { *out = make_v5_set<a, b, c_, 0>(); return true; }
+    {
+#define X(a, b, c_) if (nx == a && ny == b && nz == c_) { *out = make_v5_set<a, b, c_>(); return true; }
         LISE_MMA_SHAPES(X)
 #undef X
     }
@@ -559,14 +559,8 @@ static int abm_step(lise_ctx* c)
     const size_t slen = (size_t)4 * c->L.nxyz;
     TRY(ensure_potentials(c));                      // potentials of y_n
     const bool pipe = c->ks.v5 && c->overlap;
-    // two H-apply streams only while lise_step runs on the internal stream (both are internal, same priority)
-    const bool two = pipe && c->twostream && c->user_stream_valid && c->stream == c->streamH;
-    cudaStream_t const smain = c->stream;
     for (int phase = 1; phase <= 2; ++phase) {
         TRY(zero_partials(c, 0)); TRY(zero_partials(c, 1));
-        if (two) {                                  // the second stream starts behind the potentials of this phase
-            CK(cudaEventRecord(c->ev_h2a, smain)); CK(cudaStreamWaitEvent(c->streamH2, c->ev_h2a, 0));
-        }
         int i = 0;                                  // chunk counter across both species
         // densities of the new state: accumulated over groups of `dgroup` chunks (one launch pair per group), behind
         // the H-apply of the following chunk so that the update of the last chunk of the group overlaps it
@@ -584,15 +578,11 @@ static int abm_step(lise_ctx* c)
                 const size_t off = s0 * slen;
                 const int wb = pipe ? (i & 1) : 0;
                 const cplx* X = (phase == 1 ? S(c, q, RA) : S(c, q, RF)) + off;
-                cudaStream_t sh = (two && (i & 1)) ? c->streamH2 : smain;      // this chunk's H-apply stream
-                if (pipe && i >= 2) CK(cudaStreamWaitEvent(sh, c->ev_u[wb], 0));   // W[wb], eta[wb] are free again
-                c->stream = sh;
-                const int rch = apply_h_chunk(c, q, X, Wbuf(c, wb), etabuf(c, wb), ns);
-                c->stream = smain;
-                TRY(rch);
+                if (pipe && i >= 2) CK(cudaStreamWaitEvent(c->stream, c->ev_u[wb], 0));   // W[wb], eta[wb] are free again
+                TRY(apply_h_chunk(c, q, X, Wbuf(c, wb), etabuf(c, wb), ns));
                 UArgs u = make_uargs(c, q, off, ns, wb);
                 cudaStream_t su = pipe ? c->stream2 : c->stream;
-                if (pipe) { CK(cudaEventRecord(c->ev_h[wb], sh)); CK(cudaStreamWaitEvent(c->stream2, c->ev_h[wb], 0)); }
+                if (pipe) { CK(cudaEventRecord(c->ev_h[wb], c->stream)); CK(cudaStreamWaitEvent(c->stream2, c->ev_h[wb], 0)); }
                 if (phase == 1) TRY(launch_update<1>(c, u, su)); else TRY(launch_update<2>(c, u, su));
                 if (pipe) CK(cudaEventRecord(c->ev_u[wb], c->stream2));
                 if (c->ks.v5) {
@@ -604,10 +594,6 @@ static int abm_step(lise_ctx* c)
                 }
             }
         TRY(flush_dens(i - 1));
-        if (two) {                                  // join the second stream (its last H-apply is ordered before the last updates,
-            CK(cudaEventRecord(c->ev_h2b, c->streamH2));   // which flush_dens waited for, but make the join explicit)
-            CK(cudaStreamWaitEvent(smain, c->ev_h2b, 0));
-        }
         if (phase == 1) TRY(grid_phase(c, 1));     // potentials of the modifier m
     }
     // y_{n+1} sits in B: A <-> B; f history shifts
@@ -718,10 +704,24 @@ static int default_chunk(const lise_ctx* c)
     int ch = (int)(170.0 * 1048576.0 / sbytes);
     if (ch < c->G) ch = c->G;
     ch = (ch / c->G) * c->G;
-    if (const char* e = getenv("LISE_CHUNK")) { int v = atoi(e); if (v > 0) ch = v; }
     if (ch > nmax) ch = nmax;
     if (ch < 1) ch = 1;
     return ch;
+}
+
+// Coulomb work arrays (padded cube of side P = 3 max(N)); allocated when Coulomb is first switched on
+static int alloc_coulomb(lise_ctx* c)
+{
+    if (c->tw) return LISE_OK;
+    const Lattice& L = c->L;
+    const int P = c->P;
+    std::vector<double2> tw(P);
+    const long double pi = 3.14159265358979323846264338327950288L;
+    for (int r = 0; r < P; ++r) { long double ph = 2.0L * pi * r / P; tw[r] = make_double2((double)cosl(ph), (double)-sinl(ph)); }
+    DM(c->tw, P);
+    CK(cudaMemcpy(c->tw, tw.data(), sizeof(double2) * P, cudaMemcpyHostToDevice));
+    DM(c->cA1, (size_t)L.nx * L.ny * P); DM(c->cA2, (size_t)L.nx * P * P); DM(c->cA3, (size_t)P * P * P);
+    return LISE_OK;
 }
 
 static int ctx_init(lise_ctx* c)
@@ -730,13 +730,7 @@ static int ctx_init(lise_ctx* c)
     const size_t nx = L.nxyz;
     // blocking and launch shapes
     c->R = (L.nx % 4 == 0 && L.ny % 4 == 0 && L.nz % 4 == 0) ? 4 : 2;
-    if (const char* e = getenv("LISE_R")) {
-        int r = atoi(e);
-        if ((r == 2 || r == 4 || r == 8) && L.nx % r == 0 && L.ny % r == 0 && L.nz % r == 0) c->R = r;
-    }
-    bool want_mma = true;
-    if (const char* e = getenv("LISE_LINE_OP")) want_mma = (strcmp(e, "dense") != 0);
-    c->mma = pick_kernels(L.nx, L.ny, L.nz, c->R, want_mma, &c->ks) ? 1 : 0;
+    c->mma = pick_kernels(L.nx, L.ny, L.nz, c->R, &c->ks) ? 1 : 0;
     if (!c->mma) {
         const int ld = L.nz + 1;
         const int n1[2] = {L.ny, L.nx};
@@ -769,7 +763,6 @@ static int ctx_init(lise_ctx* c)
         const int minp = L.nx < L.ny ? L.nx : L.ny;
         c->G = (2 * nsm + minp - 1) / minp;
     }
-    if (const char* e = getenv("LISE_G")) { int g = atoi(e); if (g > 0) c->G = g; }
     if (c->G > LISE_MAXG) c->G = LISE_MAXG;
     if (c->G < 1) c->G = 1;
     c->chunk = default_chunk(c);
@@ -794,11 +787,6 @@ static int ctx_init(lise_ctx* c)
         CK(cudaDeviceGetStreamPriorityRange(&lo, &hi));
         CK(cudaStreamCreateWithPriority(&c->stream2, cudaStreamNonBlocking, lo));
         CK(cudaStreamCreateWithPriority(&c->streamH, cudaStreamNonBlocking, hi));
-        CK(cudaStreamCreateWithPriority(&c->streamH2, cudaStreamNonBlocking, hi));
-        CK(cudaEventCreateWithFlags(&c->ev_h2a, cudaEventDisableTiming));
-        CK(cudaEventCreateWithFlags(&c->ev_h2b, cudaEventDisableTiming));
-        c->twostream = 0;                   // measured: no gain on config 1 (60.7 against 60.5 ms per step); kept as an option
-        if (const char* e = getenv("LISE_TWOSTREAM")) c->twostream = atoi(e) ? 1 : 0;
         CK(cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming));
         CK(cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming));
     }
@@ -807,9 +795,7 @@ static int ctx_init(lise_ctx* c)
         CK(cudaEventCreateWithFlags(&c->ev_u[i], cudaEventDisableTiming));
     }
     c->overlap = 1;
-    if (const char* e = getenv("LISE_OVERLAP")) c->overlap = atoi(e) ? 1 : 0;
     c->dgroup = 8;
-    if (const char* e = getenv("LISE_DGROUP")) { int g = atoi(e); if (g > 0) c->dgroup = g; }
     // state slots and scratch
     for (int q = 0; q < 2; ++q)
         for (int s = 0; s < LISE_NSLOT; ++s) {
@@ -838,22 +824,14 @@ static int ctx_init(lise_ctx* c)
     // Coulomb
     int nm = L.nx; if (L.ny > nm) nm = L.ny; if (L.nz > nm) nm = L.nz;
     c->P = 3 * nm; c->Dc = sqrt(3.0) * L.dx * nm;
-    if (c->nwf[1] > 0) {
-        const int P = c->P;
-        std::vector<double2> tw(P);
-        const long double pi = 3.14159265358979323846264338327950288L;
-        for (int r = 0; r < P; ++r) { long double ph = 2.0L * pi * r / P; tw[r] = make_double2((double)cosl(ph), (double)-sinl(ph)); }
-        DM(c->tw, P);
-        CK(cudaMemcpy(c->tw, tw.data(), sizeof(double2) * P, cudaMemcpyHostToDevice));
-        DM(c->cA1, (size_t)L.nx * L.ny * P); DM(c->cA2, (size_t)L.nx * P * P); DM(c->cA3, (size_t)P * P * P);
-    }
+    if (c->par.coulomb) TRY(alloc_coulomb(c));
     c->eblocks = 64;
     DM(c->ebuf, c->eblocks * 6);
     DM(c->ovl, (size_t)(nmax > 0 ? nmax : 1) * 4);
     return LISE_OK;
 }
 
-extern "C" int lise_create(int nx, int ny, int nz, double dx, double dt, int nwf_n, int nwf_p, lise_ctx** out)
+static int create_impl(int nx, int ny, int nz, double dx, double dt, int nwf_n, int nwf_p, lise_ctx** out)
 {
     if (!out) return LISE_EINVAL;
     *out = nullptr;
@@ -882,6 +860,10 @@ extern "C" int lise_create(int nx, int ny, int nz, double dx, double dt, int nwf
     *out = c;
     return LISE_OK;
 }
+extern "C" int lise_create(int nx, int ny, int nz, double dx, double dt, int nwf_n, int nwf_p, lise_ctx** out)
+{
+    return guarded([&] { return create_impl(nx, ny, nz, dx, dt, nwf_n, nwf_p, out); });
+}
 
 extern "C" void lise_destroy(lise_ctx* c)
 {
@@ -889,9 +871,6 @@ extern "C" void lise_destroy(lise_ctx* c)
     cudaStreamSynchronize(c->stream);
     if (c->stream2) { cudaStreamSynchronize(c->stream2); cudaStreamDestroy(c->stream2); }
     if (c->streamH) { cudaStreamSynchronize(c->streamH); cudaStreamDestroy(c->streamH); }
-    if (c->streamH2) { cudaStreamSynchronize(c->streamH2); cudaStreamDestroy(c->streamH2); }
-    if (c->ev_h2a) cudaEventDestroy(c->ev_h2a);
-    if (c->ev_h2b) cudaEventDestroy(c->ev_h2b);
     if (c->ev_fork) cudaEventDestroy(c->ev_fork);
     if (c->ev_join) cudaEventDestroy(c->ev_join);
     for (int i = 0; i < 2; ++i) { if (c->ev_h[i]) cudaEventDestroy(c->ev_h[i]); if (c->ev_u[i]) cudaEventDestroy(c->ev_u[i]); }
@@ -908,6 +887,7 @@ extern "C" int lise_set_params(lise_ctx* c, const lise_params* p)
 {
     if (!c || !p) return LISE_EINVAL;
     c->par = *p;
+    if (c->par.coulomb) { const int rc = guarded([&] { return alloc_coulomb(c); }); if (rc != LISE_OK) return rc; }
     set_physconst(c);
     c->pot_valid = 0;
     return LISE_OK;
@@ -939,6 +919,13 @@ extern "C" int lise_set_overlap(lise_ctx* c, int enable)
 {
     if (!c) return LISE_EINVAL;
     c->overlap = enable ? 1 : 0;
+    return LISE_OK;
+}
+
+extern "C" int lise_set_density_group(lise_ctx* c, int nchunks)
+{
+    if (!c) return LISE_EINVAL;
+    c->dgroup = nchunks > 0 ? nchunks : 8;
     return LISE_OK;
 }
 
@@ -1031,7 +1018,7 @@ extern "C" int lise_apply_h(lise_ctx* c, int q, const void* in_dev, void* out_de
     return LISE_OK;
 }
 
-extern "C" int lise_step(lise_ctx* c, int nsteps)
+static int step_impl(lise_ctx* c, int nsteps)
 {
     if (!c || nsteps < 0) return LISE_EINVAL;
     TRY(need_both(c));
@@ -1055,8 +1042,12 @@ extern "C" int lise_step(lise_ctx* c, int nsteps)
     }
     return rc;
 }
+extern "C" int lise_step(lise_ctx* c, int nsteps)
+{
+    return guarded([&] { return step_impl(c, nsteps); });
+}
 
-extern "C" int lise_observables(lise_ctx* c, lise_observables_t* o)
+static int observables_impl(lise_ctx* c, lise_observables_t* o)
 {
     if (!c || !o) return LISE_EINVAL;
     TRY(need_both(c));
@@ -1092,6 +1083,10 @@ extern "C" int lise_observables(lise_ctx* c, lise_observables_t* o)
     o->norm_defect = nd; o->ortho_defect = od;
     o->time = c->time; o->step = c->step;
     return LISE_OK;
+}
+extern "C" int lise_observables(lise_ctx* c, lise_observables_t* o)
+{
+    return guarded([&] { return observables_impl(c, o); });
 }
 
 extern "C" int lise_profile(lise_ctx* c, int enable)
@@ -1144,40 +1139,6 @@ extern "C" int lise_measure_fp64_peak(void* stream, double seconds, double* tflo
     *tflops_host = best;
     if (sm_mhz_host) *sm_mhz_host = 0.0;
     return rc;
-}
-
-// clocks per iteration and SM sub-partition of the DMMA/DFMA mix `variant` with `warps` warps per CTA (1 CTA per SM)
-extern "C" int lise_measure_fp64_mix(int variant, int warps, double* clocks_per_iter_host)
-{
-    if (!clocks_per_iter_host || warps < 1 || warps > 12) return LISE_EINVAL;
-    int dev = 0, nsm = 0, khz = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return LISE_ECUDA;
-    cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, dev);
-    double* out = nullptr;
-    if (cudaMalloc(&out, sizeof(double) * nsm * 384) != cudaSuccess) return LISE_ENOMEM;
-    cudaEvent_t e0, e1; cudaEventCreate(&e0); cudaEventCreate(&e1);
-    const int iters = 20000;
-    float best = 1e30f;
-    for (int rep = 0; rep < 4; ++rep) {
-        cudaEventRecord(e0, 0);
-        switch (variant) {
-        case 0: k_fp64_mix<8, 0><<<nsm, 32 * warps>>>(out, iters, 0.999999, 1e-9); break;
-        case 1: k_fp64_mix<0, 16><<<nsm, 32 * warps>>>(out, iters, 0.999999, 1e-9); break;
-        case 2: k_fp64_mix<8, 8><<<nsm, 32 * warps>>>(out, iters, 0.999999, 1e-9); break;
-        case 3: k_fp64_mix<8, 16><<<nsm, 32 * warps>>>(out, iters, 0.999999, 1e-9); break;
-        case 4: k_fp64_mix<8, 32><<<nsm, 32 * warps>>>(out, iters, 0.999999, 1e-9); break;
-        case 5: k_fp64_mix<16, 0><<<nsm, 32 * warps>>>(out, iters, 0.999999, 1e-9); break;
-        default: cudaFree(out); return LISE_EINVAL;
-        }
-        cudaEventRecord(e1, 0);
-        if (cudaEventSynchronize(e1) != cudaSuccess || cudaGetLastError() != cudaSuccess) { cudaFree(out); return LISE_ECUDA; }
-        float ms = 0.f; cudaEventElapsedTime(&ms, e0, e1);
-        if (ms < best) best = ms;
-    }
-    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(out);
-    // warps are spread over the 4 sub-partitions: clocks per iteration of ONE warp's instruction bundle, per sub-partition share
-    *clocks_per_iter_host = (double)best * 1e-3 * (double)khz * 1e3 / iters;
-    return LISE_OK;
 }
 
 // host-only: the block-diagonalised tables of a line of n points (no CUDA call; tests pin them against Eqs. 49-50)

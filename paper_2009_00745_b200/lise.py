@@ -32,7 +32,7 @@ EXPORTS = ["lise_default_params", "lise_create", "lise_destroy", "lise_set_param
            "lise_set_dt", "lise_set_chunk", "lise_set_overlap", "lise_set_wavefunctions", "lise_get_wavefunctions",
            "lise_upload_wavefunctions", "lise_download_wavefunctions", "lise_set_reduce_hook",
            "lise_densities", "lise_potentials", "lise_apply_h", "lise_step", "lise_observables",
-           "lise_profile", "lise_profile_read", "lise_measure_fp64_peak", "lise_measure_fp64_mix", "lise_line_operator", "lise_line_operator_tables", "lise_launch_count", "lise_device_bytes", "lise_strerror", "lise_last_error"]
+           "lise_profile", "lise_profile_read", "lise_measure_fp64_peak", "lise_set_density_group", "lise_line_operator", "lise_line_operator_tables", "lise_launch_count", "lise_device_bytes", "lise_strerror", "lise_last_error"]
 
 
 REDUCE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_long)
@@ -56,7 +56,7 @@ def load():
     if _lib is not None:
         return _lib
     try:
-        _build.build()
+        _build.build()          # serialised across processes by a file lock; written to a temp file, then renamed
     except Exception as exc:  # nvcc missing on the box: use the shipped .so if there is one
         if not os.path.exists(_build.SO):
             raise RuntimeError(f"liblise.so is missing and could not be built: {exc}") from exc
@@ -84,7 +84,7 @@ def load():
     lib.lise_profile_read.argtypes = [vp, C.POINTER(dp), C.POINTER(C.c_long)]
     lib.lise_measure_fp64_peak.argtypes = [vp, dp, C.POINTER(dp), C.POINTER(dp)]
     lib.lise_line_operator.argtypes = [vp]; lib.lise_line_operator.restype = C.c_char_p
-    lib.lise_measure_fp64_mix.argtypes = [ip, ip, C.POINTER(dp)]
+    lib.lise_set_density_group.argtypes = [vp, ip]
     lib.lise_line_operator_tables.argtypes = [ip, dp, C.POINTER(dp), ip, C.POINTER(ip)]
     lib.lise_launch_count.argtypes = [vp]; lib.lise_launch_count.restype = C.c_long
     lib.lise_device_bytes.argtypes = [vp]; lib.lise_device_bytes.restype = C.c_longlong
@@ -128,6 +128,18 @@ def line_operator_tables(n, dx):
     return dict(H=H, R=R, J=J, ND=ND), tab.reshape(2, J, 2, ND)
 
 
+def capacity_states(shape, free_bytes, requested, reserve_bytes=6 * 2 ** 30, multiple=256):
+    """capacity rule of SURVEY 8(d) / Appendix C: the library keeps 7 state arrays of S = 64 Nxyz bytes per state
+    (+ a chunk-sized H psi scratch and grid fields, covered by `reserve_bytes`).  Returns the (n, p) state counts that
+    fit `free_bytes` of device memory: `requested` if it fits, else the largest multiple of `multiple` per species."""
+    S = 64 * shape[0] * shape[1] * shape[2]
+    cap = int((free_bytes - reserve_bytes) // (7 * S))
+    if requested[0] + requested[1] <= cap:
+        return tuple(requested)
+    each = max(multiple, (cap // 2) // multiple * multiple)
+    return (min(requested[0], each), min(requested[1], each))
+
+
 class LiseError(RuntimeError):
     pass
 
@@ -151,11 +163,18 @@ class Lise:
             self._h = C.c_void_p()
             raise LiseError(f"lise_create failed: {self.lib.lise_strerror(rc).decode()} ({rc})")
         st = torch.cuda.current_stream(self.device) if stream is None else stream
+        self._stream_ptr = st.cuda_stream
         self._chk(self.lib.lise_set_stream(self._h, C.c_void_p(st.cuda_stream)), "lise_set_stream")
+        self.params = default_params()
+        if nwf_p == 0:
+            self.params.coulomb = 0            # lise_create's default for a context without proton states
         if params is not None:
             self.set_params(params)
 
     def _chk(self, rc, what):
+        if rc != 0 and getattr(self, "_hook_error", None) is not None:
+            exc, self._hook_error = self._hook_error, None
+            raise LiseError(f"{what} failed in the reduce hook: {exc!r}") from exc
         if rc != 0:
             msg = self.lib.lise_last_error(self._h).decode() if self._h else ""
             raise LiseError(f"{what} failed: {self.lib.lise_strerror(rc).decode()} ({rc}) {msg}")
@@ -178,10 +197,15 @@ class Lise:
         return C.c_void_p(t.data_ptr())
 
     def set_params(self, params):
+        self.params = params
         self._chk(self.lib.lise_set_params(self._h, C.byref(params)), "lise_set_params")
 
     def set_stream(self, stream):
+        self._stream_ptr = stream.cuda_stream
         self._chk(self.lib.lise_set_stream(self._h, C.c_void_p(stream.cuda_stream)), "lise_set_stream")
+
+    def set_density_group(self, nchunks):
+        self._chk(self.lib.lise_set_density_group(self._h, nchunks), "lise_set_density_group")
 
     def set_dt(self, dt):
         self.dt = dt
@@ -229,7 +253,9 @@ class Lise:
 
         def _cb(user, ptr, count):
             try:
-                reduce_tensor(torch.as_tensor(_DevView(ptr, count), device=self.device))
+                # lise.h: the reduction must be enqueued on the CONTEXT's stream, which need not be torch's current one
+                with torch.cuda.device(self.device), torch.cuda.stream(torch.cuda.ExternalStream(self._stream_ptr, device=self.device)):
+                    reduce_tensor(torch.as_tensor(_DevView(ptr, count), device=self.device))
                 return 0
             except Exception as exc:  # never let an exception cross the C ABI
                 self._hook_error = exc
@@ -283,3 +309,20 @@ class Lise:
 
     def device_bytes(self):
         return int(self.lib.lise_device_bytes(self._h))
+
+
+def _on_device(method):
+    """run a Lise method with the context's device current (the C library launches on the current device)."""
+    import functools
+
+    @functools.wraps(method)
+    def wrapper(self, *a, **k):
+        with torch.cuda.device(self.device):
+            return method(self, *a, **k)
+    return wrapper
+
+
+for _name in ("close", "set_params", "set_stream", "set_density_group", "set_dt", "set_chunk", "set_overlap",
+              "set_wavefunctions", "get_wavefunctions", "upload_wavefunctions", "download_wavefunctions",
+              "set_reduce_hook", "densities", "potentials", "apply_h", "step", "observables", "profile", "profile_read"):
+    setattr(Lise, _name, _on_device(getattr(Lise, _name)))

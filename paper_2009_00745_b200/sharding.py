@@ -32,8 +32,15 @@ def allreduce_sum_(t, group=None):
     return t
 
 
-def attach(ctx, group=None):
-    """make `ctx` (paper_2009_00745_b200.lise.Lise) sum its density accumulators over the ranks of `group`."""
+def attach(ctx, group=None, global_nwf=None, coulomb=True):
+    """make `ctx` (paper_2009_00745_b200.lise.Lise) sum its density accumulators over the ranks of `group`.
+    global_nwf = (neutron, proton) state counts over all ranks: Coulomb is decided from the GLOBAL proton count, so
+    that a rank that happens to own no proton state still computes the same potentials and energy as the others."""
+    if global_nwf is not None:
+        want = 1 if (global_nwf[1] > 0 and coulomb) else 0
+        if ctx.params.coulomb != want:
+            ctx.params.coulomb = want
+            ctx.set_params(ctx.params)
     ctx.set_reduce_hook(lambda t: allreduce_sum_(t, group))
 
 

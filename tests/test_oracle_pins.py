@@ -549,8 +549,9 @@ def test_energy_number_conserved_pairing_off_and_time_reversal():
 
 
 def test_starter_is_third_order():
-    """the 3 starter steps (midpoint Hamiltonian) have a global error O(dt^3): halving dt divides the
-    difference to a fine reference by about 8-9 (reading B18)."""
+    """starter only (3 series-expansion steps with the midpoint Hamiltonian, Eqs. 75-77, reading B18): the error after
+    the 3 steps against a fine reference at the same final time is O(dt^3); halving dt divides it by 8-9 (SURVEY 8(c)
+    states an observed ratio of about 9)."""
     from paper_2009_00745_b200 import inputs
     cfg = dict(inputs.CONFIGS[0]); cfg["shape"] = (6, 6, 6); cfg["dx"] = 1.5
     psi = inputs.make_species(cfg, 0, 6, seed=3).numpy()
@@ -558,10 +559,11 @@ def test_starter_is_third_order():
     def run(dt, n):
         c = ref.RefContext(*cfg["shape"], cfg["dx"], dt, 6, 0)
         c.set_wavefunctions(0, psi); c.step(n)
-        return c.densities(0)[0]
+        w = c.get_wavefunctions(0); c.close()
+        return w
 
-    T = 0.6
-    fine = run(T / 24, 24)
-    e1 = np.abs(run(T / 3, 3) - fine).max()
-    e2 = np.abs(run(T / 6, 6) - fine).max()   # 3 starter + 3 ABM steps
-    assert e2 < e1 / 4
+    def starter_error(dt):
+        return np.abs(run(dt, 3) - run(3 * dt / 48, 48)).max()
+
+    e1, e2 = starter_error(0.2), starter_error(0.1)
+    assert 7.0 < e1 / e2 < 10.0, (e1, e2, e1 / e2)
