@@ -185,6 +185,10 @@ def run_ours(args):
     g = lise.Lise(*shape, cfg["dx"], cfg["dt"], nwf[0], nwf[1])
     if world > 1:
         sharding.attach(g)
+    if args.chunk:
+        g.set_chunk(args.chunk)
+    if args.dgroup:
+        g.set_density_group(args.dgroup)
     host = []
     for q in (0, 1):
         first = rank * nwf[q]
@@ -236,7 +240,7 @@ def run_ours(args):
     g.step(max(1, min(args.steps, 2)))
     prof = g.profile_read()
     g.profile(False)
-    g.set_overlap(os.environ.get("LISE_OVERLAP", "1") != "0")
+    g.set_overlap(True)
     psteps = max(1, min(args.steps, 2))
 
     # ---- end to end through the C-ABI with HOST buffers ----
@@ -383,6 +387,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=1, help="index into BASELINE.json configs (default 1: the 24^3 workload)")
     ap.add_argument("--nwf", type=int, nargs=2, default=None, help="override states per species per GPU (testing)")
+    ap.add_argument("--chunk", type=int, default=0, help="states per kernel launch (0 = the library's default)")
+    ap.add_argument("--dgroup", type=int, default=0, help="chunks per density launch (0 = the library's default)")
     ap.add_argument("--no-e2e", dest="e2e", action="store_false")
     ap.add_argument("--no-cpu-baseline", dest="cpu_baseline", action="store_false")
     ap.add_argument("--cpu-states", type=int, default=0, help="oracle sample: states per species (0 = sized from the host core count)")

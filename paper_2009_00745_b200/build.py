@@ -13,8 +13,22 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", 
 
 
 def _deps():
-    return (glob.glob(os.path.join(CSRC, "*.cu")) + glob.glob(os.path.join(CSRC, "*.cuh"))
+    return ([f for f in glob.glob(os.path.join(CSRC, "*.cu")) + glob.glob(os.path.join(CSRC, "*.cuh"))
+             if not f.endswith("line_codelets.cuh")]
             + glob.glob(os.path.join(CSRC, "*.py")) + [os.path.join(HERE, "..", "include", "lise.h")])
+
+
+def _codelets():
+    """(re)generate csrc/line_codelets.cuh, the straight-line FFT code of the line operators, from gen_codelets.py"""
+    gen = os.path.join(CSRC, "gen_codelets.py")
+    out = os.path.join(CSRC, "line_codelets.cuh")
+    if os.path.exists(out) and os.path.getmtime(out) >= os.path.getmtime(gen):
+        return
+    import importlib.util
+    spec = importlib.util.spec_from_file_location("lise_gen_codelets", gen)
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    mod.generate(out)
 
 
 def needs_build():
@@ -34,6 +48,7 @@ def build(force=False, verbose=False):
         try:
             if not force and not needs_build():      # another process built it while we waited
                 return SO
+            _codelets()
             nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
             tmp = SO + f".tmp{os.getpid()}"
             cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SOURCES

@@ -351,7 +351,16 @@ def schedule(d, outs):
                 fused[n] = 0
     nadd = nmul = nfma = 0
     order = []
+    depth = {}
     for n in sorted(live):
+        k = d.kind[n]
+        if k == "in":
+            depth[n] = 0
+        elif k == "mul":
+            depth[n] = depth[d.args[n][1]] + (1 if n in standalone else 0)
+        else:
+            depth[n] = 1 + max(depth[d.args[n][0]], depth[d.args[n][1]])
+    for n in sorted(live, key=lambda v: (depth[v], v)):
         k = d.kind[n]
         if k == "in":
             continue
