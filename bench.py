@@ -37,11 +37,12 @@ def read_peaks():
 
 
 def measured_traffic(cls, workload, states_per_launch):
-    """DRAM bytes per launch of kernel class `cls` from the committed ncu capture (profiles/r1_v5_traffic.md: bytes per
-    state on the config-1 lattice), or None for other workloads / when the file is absent."""
+    """DRAM bytes per launch of kernel class `cls` from the committed ncu capture (profiles/r2_traffic.md: bytes per
+    state on the config-1 lattice, `ncu --set full`, dram__bytes_read.sum + dram__bytes_write.sum), or None for other
+    workloads / when the file is absent.  Not measured in this run: a number taken under ncu is never a bench value."""
     if not workload.startswith("config1"):
         return None
-    path = os.path.join(ROOT, "profiles", "r1_v5_traffic.md")
+    path = os.path.join(ROOT, "profiles", "r2_traffic.md")
     try:
         for line in open(path):
             cells = [c.strip() for c in line.strip().strip("|").split("|")]
@@ -106,19 +107,34 @@ def workload(idx, nwf_override=None):
     return cfg, nwf
 
 
-def make_shard(cfg, q, nwf_total, first, count, seed, device):
-    """this rank's states of species q: occupancy from the GLOBAL count, orthonormalised within the shard."""
-    import torch
-    from paper_2009_00745_b200 import inputs
-    if count == 0:
-        return torch.zeros((0, 4) + tuple(cfg["shape"]), dtype=torch.complex128, device=device)
-    return inputs.make_block(cfg, q, nwf_total, first, count, seed, device)
+# ---- ALGORITHMIC work per kernel class, per state and evaluation (two evaluations per ABM step) ----
+# flops: an axis pass = one 1-D transform of every line of one component along one axis = 5 N log2 N per line of N
+# points, i.e. 5 log2 N per lattice point.  H-apply: 4 components x 6 passes per axis (inner 1 forward + 2 inverse,
+# outer 2 forward + 1 inverse); densities: 2 v-components x 3 passes per axis; pointwise: 545 (H-apply incl. the k-space
+# multipliers and pairing, two thirds on the yz kernel), 120 (density accumulators, same split), 16 (eta), 270 per STEP
+# for the ABM linear combinations.  Sum over a step = 300 (log2 Nx + log2 Ny + log2 Nz) + 1600 per point, the survey's figure.
+# bytes: 15 S per step (S = 64 Nxyz): X read once per evaluation (charged to the yz kernel), phase 1: 5 history reads
+# + 4 writes, phase 2: 2 reads + 2 writes (charged to the update).  W = H psi is NOT counted: it should stay on chip.
+def algorithmic_model(shape):
+    lx, ly, lz = (math.log2(n) for n in shape)
+    return {
+        "happly_yz": dict(flop=4 * 6 * 5.0 * (ly + lz) + 545.0 * 2 / 3, S=1.0),
+        "happly_xz": dict(flop=4 * 6 * 5.0 * lx + 545.0 / 3 + 16.0, S=0.0),
+        "update": dict(flop=135.0, S=6.5),                          # mean of 9 S (evaluation 1) and 4 S (evaluation 2)
+        "dens_yz": dict(flop=2 * 3 * 5.0 * (ly + lz) + 120.0 * 2 / 3, S=0.0),
+        "dens_x": dict(flop=2 * 3 * 5.0 * lx + 120.0 / 3, S=0.0),
+        "grid": dict(flop=0.0, S=0.0),
+    }
 
 
-# per-kernel-class algorithmic traffic in units of one state array S = 64 Nxyz bytes per state processed, and
-# fp64-pipe work (FMA-equivalents: 256 per DMMA m8n8k4, 1 per DFMA) per lattice point per state processed
-# (DESIGN.md section 6, kernel table).  Block-diagonalised circulant: a line of N = 8 R points costs
-# dmma(N) = 2 (real blocks) + 8 (conjugate pairs) tiles per 8 real columns and operator application.
+def step_flops_per_point(shape):
+    return 300.0 * sum(math.log2(n) for n in shape) + 1600.0
+
+
+# ---- EXECUTED fp64-pipe work of this build (a model of what the kernels run, not the roofline numerator) ----
+# FFT line operator: the generated codelets' instruction counts (lise_line_operator_cost: inner + outer per real line
+# of N points = 4 operator applications on one real part); DMMA line operator: 256 FMA slots per m8n8k4 tile,
+# dmma_tiles(N) tiles per 8 real columns and operator application; + pointwise slots.  1 slot = 1 fp64 instruction lane.
 def dmma_tiles(n):
     if n % 8 == 0 and 16 <= n <= 64:
         r = n // 8
@@ -127,79 +143,74 @@ def dmma_tiles(n):
     return ((n + 7) // 8) * (n // 4)                               # plain circulant
 
 
-def line_fma_per_point(n):
-    """DMMA FMAs per complex lattice point for ONE operator application along a line of n points."""
-    return dmma_tiles(n) * 256.0 / (4.0 * n)                       # a tile covers 4 complex lines (8 real columns)
-
-
-def class_model(shape, line_op):
+def executed_model(shape, line_op, lise):
     nx, ny, nz = shape
-    if line_op == "dense":
-        fx, fy, fz = (2.0 * n for n in (nx, ny, nz))                 # DFMA circulant sums: 2 N per complex point
-    else:
-        fx, fy, fz = (line_fma_per_point(n) for n in (nx, ny, nz))
-    pw_h = 50.0                                                    # pointwise FMAs per point, component and axis (B, M products, real DFT)
+
+    def dmma_axis(n):                                              # slots per complex point, component and axis (4 applications)
+        return 4 * dmma_tiles(n) * 256.0 / (4.0 * n)
+
+    def fft_axis(n):
+        c = lise.line_operator_cost(n)
+        return 2.0 * (c[0] + c[1]) / n if c[0] else dmma_axis(n)
+    pw = 50.0                                                      # pointwise + small transforms per point, component and axis
+    fft_yz = line_op == "fft"
+    fft_xz = fft_yz and max(ny, nz) > 24                           # the xz kernel is the FFT one only on 2-spinor-unit lattices
+    ay = (fft_axis if fft_yz else dmma_axis)
+    ax = (fft_axis if fft_xz else dmma_axis)
     return {
-        "happly_yz": dict(S=2.0, slots=4 * (4 * (fy + fz) + 2 * pw_h) + 4 * 12),   # read X, write W
-        "happly_xz": dict(S=3.0, slots=4 * (4 * fx + pw_h)),                       # read X, W; write W
-        "update": dict(S=8.5, slots=40.0),                         # evaluation 1: 7 + 4 S, evaluation 2: 4 + 2 S -> mean 8.5
-        "dens_yz": dict(S=0.75, slots=2 * (2 * (fy + fz) + 20) + 20),              # read v_up, v_dn, u_up of the new state
-        "dens_x": dict(S=0.5, slots=2 * (2 * fx + 10)),            # read v_up, v_dn of the new state
-        "grid": dict(S=0.0, slots=0.0),
+        "happly_yz": 4 * (ay(ny) + ay(nz) + 2 * pw) + 4 * 12,
+        "happly_xz": 4 * (ax(nx) + pw),
+        "update": 40.0,
+        "dens_yz": 2 * (0.5 * (dmma_axis(ny) + dmma_axis(nz)) + 20) + 20,
+        "dens_x": 2 * (0.5 * dmma_axis(nx) + 10),
+        "grid": 0.0,
     }
 
 
-def run_ours(args):
+def run_workload(args, cfg_idx, nwf_req, env, primary):
+    """one workload on this rank's GPU: setup, starter, warm-up, K timed ABM steps, per-class times; returns a dict
+    (rank 0) or None."""
     import torch
     import torch.distributed as dist
     from paper_2009_00745_b200 import inputs, lise, sharding
-
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback (use --impl reference for the oracle)")
-    torch.cuda.set_device(local)
-    dev = torch.device("cuda", local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
-    if args.gpus != world and rank == 0:
-        print(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}; using {world}", file=sys.stderr)
-
-    cfg, nwf = workload(args.config, args.nwf)
+    world, rank, dev, local = env["world"], env["rank"], env["dev"], env["local"]
+    cfg, nwf = workload(cfg_idx, nwf_req)
     shape = tuple(cfg["shape"]); nxyz = shape[0] * shape[1] * shape[2]
     S = 64.0 * nxyz
-    # capacity rule (SURVEY 8(d)): 7 resident state arrays + scratch must fit; shrink to a multiple of 256 if not
-    free, total = torch.cuda.mem_get_info(dev)
-    # 7 resident arrays + one species' input block and its orthonormalisation workspace while the inputs are generated
-    per_state = 9 * S
-    cap = int((free - 12 * 2 ** 30) / per_state)
+    torch.cuda.empty_cache()
+    free, _ = torch.cuda.mem_get_info(dev)
     req = nwf
-    if nwf[0] + nwf[1] > cap:
-        each = max(256, (cap // 2) // 256 * 256)
-        nwf = (min(nwf[0], each), min(nwf[1], each))
-    tot = (nwf[0] * world, nwf[1] * world)                      # weak scaling: global counts
-    seed = inputs.SEED0 + args.config
+    nwf = lise.capacity_states(shape, free, nwf)                 # SURVEY 8(d) / Appendix C: 7 state arrays must fit
+    tot = (nwf[0] * world, nwf[1] * world)                        # weak scaling: global counts
+    seed = inputs.SEED0 + cfg_idx
+    steps = args.steps if primary else max(2, min(args.steps, 3))
 
+    # inputs first, parked in pinned host memory: the generator's workspace and the context's 7 arrays do not fit side
+    # by side at capacity; the host copies are also the end-to-end leg's mirror
     t0 = time.time()
+    host = []
+    for q in (0, 1):
+        if nwf[q] == 0:
+            host.append(None)
+            continue
+        psi = inputs.make_block(cfg, q, tot[q], rank * nwf[q], nwf[q], seed, dev)
+        h = torch.empty(psi.shape, dtype=torch.complex128, pin_memory=True)
+        h.copy_(psi)
+        host.append(h)
+        del psi
+    torch.cuda.empty_cache()
     g = lise.Lise(*shape, cfg["dx"], cfg["dt"], nwf[0], nwf[1])
     if world > 1:
-        sharding.attach(g)
+        sharding.attach(g, global_nwf=tot, coulomb=bool(cfg["coulomb"]))
     if args.chunk:
         g.set_chunk(args.chunk)
     if args.dgroup:
         g.set_density_group(args.dgroup)
-    host = []
     for q in (0, 1):
-        first = rank * nwf[q]
-        psi = make_shard(cfg, q, tot[q], first, nwf[q], seed, dev)
-        g.set_wavefunctions(q, psi)
-        if args.e2e and nwf[q]:
-            h = torch.empty(psi.shape, dtype=torch.complex128, pin_memory=True)
-            host.append(h)
+        if host[q] is not None:
+            g.upload_wavefunctions(q, host[q])
         else:
-            host.append(None)
-        del psi
+            g.set_wavefunctions(q, torch.zeros((0, 4) + shape, dtype=torch.complex128, device=dev))
     torch.cuda.synchronize()
     t_setup = time.time() - t0
 
@@ -218,7 +229,7 @@ def run_ours(args):
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     wall0 = time.time()
     ev0.record()
-    g.step(args.steps)
+    g.step(steps)
     ev1.record()
     barrier()
     wall = time.time() - wall0
@@ -229,29 +240,29 @@ def run_ours(args):
         t = torch.tensor([ms], dtype=torch.float64, device=dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms = float(t[0])
-    value = nstates * world * args.steps / (ms * 1e-3)
+    value = nstates * world * steps / (ms * 1e-3)
     obs = g.observables()
 
     # ---- per-kernel-class device times (CUDA events inside the library, on the launching stream) ----
     # with the two-stream overlap off: a class time is then that kernel running alone, which is what a per-kernel
     # roofline needs (overlapped, the update and the H-apply kernels share SMs and stretch each other)
+    psteps = max(1, min(steps, 2))
     g.set_overlap(False)
     g.profile(True)
-    g.step(max(1, min(args.steps, 2)))
+    g.step(psteps)
     prof = g.profile_read()
     g.profile(False)
     g.set_overlap(True)
-    psteps = max(1, min(args.steps, 2))
 
     # ---- end to end through the C-ABI with HOST buffers ----
     e2e = None
-    if args.e2e:
+    if args.e2e and primary:
         for q in (0, 1):
             if host[q] is not None:
                 g.download_wavefunctions(q, host[q])            # host mirror of y_n
         barrier()
         w0 = time.time()
-        for _ in range(args.steps):
+        for _ in range(steps):
             for q in (0, 1):
                 if host[q] is not None:
                     g.upload_wavefunctions(q, host[q], keep_history=True)   # H2D of the step's input
@@ -266,63 +277,114 @@ def run_ours(args):
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             w = float(t[0])
         nbytes = sum(h.numel() * 16 for h in host if h is not None)
-        e2e = {"value": nstates * world * args.steps / w, "unit": UNIT,
+        e2e = {"value": nstates * world * steps / w, "unit": UNIT,
                "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes}
-
+    del host
+    line_op = g.line_operator()
     if rank != 0:
         g.close()
-        if world > 1:
-            dist.destroy_process_group()
-        return
+        return None
 
-    # ---- rooflines ----
+    # ---- rooflines: algorithmic flops and bytes over the measured peaks ----
     hbm_gbs, hbm_src = read_peaks()
-    fp64_tf = lise.measure_fp64_peak(1.5)
-    line_op = g.line_operator()
-    model = class_model(shape, line_op)
+    fp64_tf = env["fp64_tf"]
+    alg = algorithmic_model(shape)
+    exe = executed_model(shape, line_op, lise)
     tot_ms = sum(v[0] for v in prof.values())
     top = max((k for k in prof if k != "grid"), key=lambda k: prof[k][0])
     top_ms, top_n = prof[top]
     states_per_launch = nstates * psteps * 2.0 / max(top_n, 1)       # every state passes each class twice per step
-    bytes_per_launch = model[top]["S"] * S * states_per_launch
-    slots_per_launch = model[top]["slots"] * nxyz * states_per_launch
+    flop_per_launch = alg[top]["flop"] * nxyz * states_per_launch
+    bytes_per_launch = alg[top]["S"] * S * states_per_launch
     avg_s = top_ms * 1e-3 / max(top_n, 1)
     t_hbm = bytes_per_launch / (hbm_gbs * 1e9)
-    t_alu = slots_per_launch * 2.0 / (fp64_tf * 1e12)
-    if t_alu > t_hbm:
-        roof = {"bound": "alu", "achieved": slots_per_launch * 2.0 / avg_s * 1e-12, "peak": fp64_tf, "unit": "TFLOP/s",
-                "peak_source": "measured here: DFMA microbenchmark (lise_measure_fp64_peak), 2 flop per fp64 pipe slot"}
+    t_alu = flop_per_launch / (fp64_tf * 1e12)
+    if t_alu >= t_hbm:
+        roof = {"bound": "alu", "achieved": flop_per_launch / avg_s * 1e-12, "peak": fp64_tf, "unit": "TFLOP/s",
+                "peak_source": "measured here: DFMA microbenchmark (lise_measure_fp64_peak), 2 flop per fp64 pipe slot; "
+                               "nominal 148 SM x 64 FMA/clk x 2 x 1.965 GHz = 37.2",
+                "numerator": "SURVEY 8(d) algorithmic flops (5 N log2 N per line transform + pointwise), not executed work"}
     else:
         roof = {"bound": "hbm", "achieved": bytes_per_launch / avg_s * 1e-9, "peak": hbm_gbs, "unit": "GB/s",
-                "peak_source": hbm_src}
+                "peak_source": hbm_src, "numerator": "SURVEY 8(d) algorithmic bytes"}
     roof["frac"] = roof["achieved"] / roof["peak"]
     roof["kernel"] = top
     roof["avg_launch_ms"] = avg_s * 1e3
     roof["share_of_step"] = top_ms / tot_ms if tot_ms > 0 else None
+    roof["executed_tflops"] = exe[top] * 2.0 * nxyz * states_per_launch / avg_s * 1e-12
+    roof["executed_note"] = "model of the fp64-pipe slots this build executes (codelet / DMMA tile counts), 2 flop per slot"
     roof["traffic"] = measured_traffic(top, cfg["name"], states_per_launch)
+    roof["traffic_source"] = "profiles/r2_traffic.md (committed ncu --set full capture, bytes per state x states per launch)"
     roof["classes_ms_per_step"] = {k: v[0] / psteps for k, v in prof.items()}
+    roof["classes_frac_of_fp64_peak"] = {k: (alg[k]["flop"] * nxyz * nstates * 2.0 / (v[0] / psteps * 1e-3) / (fp64_tf * 1e12)
+                                             if v[0] > 0 else None) for k, v in prof.items()}
     roof["classes_note"] = "per-class device time with the update/H-apply stream overlap off; the timed region runs with it on"
     step_bytes = 15.0 * S                                              # B_min = 960 Nxyz per qpwf-update
+    step_flop = step_flops_per_point(shape) * nxyz
     per_gpu = value / world
-    step_roof = {"hbm_bytes_per_update": step_bytes, "hbm_frac_of_measured": per_gpu * step_bytes / (hbm_gbs * 1e9),
-                 "hbm_frac_of_8TBs": per_gpu * step_bytes / 8e12, "hbm_peak_gbs": hbm_gbs, "hbm_peak_source": hbm_src,
-                 "fp64_peak_tflops_measured": fp64_tf}
-
-    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-           "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-           "dtype": "f64", "data": "synthetic",
+    hbm_frac = per_gpu * step_bytes / (hbm_gbs * 1e9)
+    fp64_frac = per_gpu * step_flop / (fp64_tf * 1e12)
+    step_roof = {"hbm_bytes_per_update": step_bytes, "flop_per_update": step_flop,
+                 "hbm_frac_of_measured": hbm_frac, "hbm_frac_of_8TBs": per_gpu * step_bytes / 8e12,
+                 "fp64_frac_of_measured": fp64_frac, "fp64_frac_of_nominal_37.2": per_gpu * step_flop / 37.2e12,
+                 "headline_frac": min(hbm_frac, fp64_frac),
+                 "headline_note": "SURVEY 8(d): min(HBM fraction, fp64 fraction) of the whole step, both of measured peaks",
+                 "hbm_peak_gbs": hbm_gbs, "hbm_peak_source": hbm_src, "fp64_peak_tflops_measured": fp64_tf}
+    par = "single GPU"
+    if world > 1:
+        par = (f"state-sharded x{world}, weak scaling: every rank owns {nstates} states, each shard orthonormalised on its "
+               "own (the union is not one orthonormal set; densities are additive either way)")
+    out = {"value": value, "ms_per_step": ms / steps, "steps": steps,
            "config": {"workload": cfg["name"], "lattice": list(shape), "dx_fm": cfg["dx"], "dt_fm_c": cfg["dt"],
-                      "states_per_gpu": list(nwf), "states_requested": list(req), "coulomb": bool(cfg["coulomb"] and nwf[1] > 0),
-                      "parallelism": f"state-sharded x{world}" if world > 1 else "single GPU",
+                      "states_per_gpu": list(nwf), "states_requested": list(req), "coulomb": bool(cfg["coulomb"] and tot[1] > 0),
+                      "parallelism": par,
                       "l2": "inputs larger than L2 (7 state arrays = %.1f GB resident)" % (7 * S * nstates / 1e9),
                       "line_operator": line_op, "setup_s": round(t_setup, 1)},
            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roof, "step_roofline": step_roof,
            "wall_s_timed_region": wall,
            "observables": {k: obs[k] for k in ("energy", "n_neutron", "n_proton", "norm_defect", "ortho_defect", "step")}}
-    if args.cpu_baseline and world == 1:
-        out["cpu_baseline"] = cpu_baseline(cfg, args.cpu_states)
     g.close()
-    print(json.dumps(out))
+    return out
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2009_00745_b200 import lise
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    if args.gpus != world and rank == 0:
+        print(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}; using {world}", file=sys.stderr)
+    env = dict(world=world, rank=rank, local=local, dev=dev, fp64_tf=lise.measure_fp64_peak(1.5) if rank == 0 else 0.0)
+    res = run_workload(args, args.config, args.nwf, env, primary=True)
+    also = []
+    if args.also and args.nwf is None:
+        for idx in args.also:
+            if idx != args.config:
+                r = run_workload(args, idx, None, env, primary=False)
+                if r is not None:
+                    also.append(r)
+    if rank == 0:
+        out = {"metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+               "ms_per_step": res["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+               "dtype": "f64", "data": "synthetic"}
+        for k in ("config", "clocks", "e2e", "gpu_launches", "roofline", "step_roofline", "wall_s_timed_region", "observables"):
+            out[k] = res[k]
+        # the other workload the target names (32^3), same invocation: its own clocks, rooflines, state counts
+        out["also"] = [{"metric": METRIC, "unit": UNIT, **{k: r[k] for k in ("value", "ms_per_step", "steps", "config", "clocks",
+                        "gpu_launches", "roofline", "step_roofline", "observables")}} for r in also]
+        if args.cpu_baseline and world == 1:
+            from paper_2009_00745_b200 import inputs
+            out["cpu_baseline"] = cpu_baseline(dict(inputs.CONFIGS[args.config]), args.cpu_states)
+        print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
 
@@ -389,6 +451,8 @@ def main():
     ap.add_argument("--nwf", type=int, nargs=2, default=None, help="override states per species per GPU (testing)")
     ap.add_argument("--chunk", type=int, default=0, help="states per kernel launch (0 = the library's default)")
     ap.add_argument("--dgroup", type=int, default=0, help="chunks per density launch (0 = the library's default)")
+    ap.add_argument("--also", type=int, nargs="*", default=[2],
+                    help="further configs timed in the same invocation and reported under \"also\" (default: 2, the 32^3 workload)")
     ap.add_argument("--no-e2e", dest="e2e", action="store_false")
     ap.add_argument("--no-cpu-baseline", dest="cpu_baseline", action="store_false")
     ap.add_argument("--cpu-states", type=int, default=0, help="oracle sample: states per species (0 = sized from the host core count)")

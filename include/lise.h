@@ -156,10 +156,15 @@ int lise_profile_read(lise_ctx *ctx, double *ms, long *counts);
  * (HOST pointer).  sm_mhz_host is reserved (set to 0).  Synchronises. */
 int lise_measure_fp64_peak(void *stream, double seconds, double *tflops_host, double *sm_mhz_host);
 
-/* Which line operator the per-state kernels of this context use: "dmma" (fp64 tensor-core tiles, for the
- * lattice shapes the library was instantiated for)
- * or "dense" (generic DFMA circulant sums, any even lattice).  Both apply the same operator (Eq. 48). */
+/* Which line operator the H-apply kernels of this context use: "fft" (one real line per thread, generated
+ * real-input FFT code, Eqs. 49-50; lattices with every edge in {8, 12, 16, 20, 24, 32}), "dmma" (block-diagonalised
+ * circulant on fp64 tensor-core tiles; the other lattice shapes the library was instantiated for) or "dense" (generic
+ * DFMA circulant sums, any even lattice).  All three apply the same operator (Eqs. 48-50). */
 const char *lise_line_operator(const lise_ctx *ctx);
+/* Host-only: the number of fp64 instructions (DADD + DMUL + DFMA) of the generated straight-line FFT code for one
+ * REAL line of n points: inner = (a = D x, b = D2 x), outer = (c = D g + D2 q); both 0 if no code was generated for n.
+ * bench.py uses them for its model of the executed (as opposed to algorithmic) fp64 work. */
+int lise_line_operator_cost(int n, int *inner_ops_host, int *outer_ops_host);
 
 /* Host-only (no CUDA call, works without a GPU): the block-diagonalised form of the lattice derivative matrices
  * D (Eq. 48a) and D2 (Eq. 48b, prefactor as DESIGN.md B3) of a periodic line of n points (n % 4 == 0) that the

@@ -32,7 +32,25 @@ typedef struct {
     double t0, t1, t2, t3, x0, x1, x2, x3, gamma, W0; /* Skyrme set (default SLy4) */
     double g0_n, g0_p;                               /* bare pairing couplings, MeV fm^3; 0 = off */
     int coulomb, pairing_rearrangement, remove_phase;
+    /* functional and pairing variants (Eqs. 8, 10, 15, 20; defaults: all off / zero) */
+    double alpha_pair;                               /* Eq. 8: g0(r) = g0 (1 - alpha n(r) / n0), n = n_n + n_p, n0 = 0.16 fm^-3 */
+    double mu_n, mu_p, e_cut;                        /* Eq. 20: chemical potentials and energy cutoff E_c (MeV), spherical cutoff */
+    double sea_a[3], sea_b[3], sea_c[3];             /* Eq. 10: SeaLL1 volume coefficients a_j, b_j, c_j (ref. [36]: not printed) */
+    double sea_cdn[2], sea_cdj[2];                   /* SeaLL1: C_t^{n Delta n}, C_t^{nabla J}, t = 0, 1 */
+    int functional;                                  /* 0 Skyrme (Eq. 9), 1 SeaLL1 (Eq. 10) */
+    int pairing_cutoff;                              /* 0 lattice cutoff (Eq. 21), 1 spherical cutoff (Eq. 20) */
+    int renormalize;                                 /* 1: every qpwf is normalised at the end of each step (L637) */
 } lise_ref_params;
+
+/* Eqs. 37-41 and the energy of the external terms; coordinates x_i = i dx (Eq. 43), Q_lm about the total c.m. */
+typedef struct {
+    double rcm[3], rcm_n[3], rcm_p[3];               /* Eq. 37, fm */
+    double q20, q30, q40, q21[2], q22[2];            /* Eq. 38 b-e of the total density (re, im for m != 0) */
+    double delta_n, delta_p;                         /* Eq. 39, MeV */
+    double e_coll;                                   /* Eq. 40 read as sum_q int (hbar^2/2m) j_q^2 / n_q, MeV */
+    double v_cm[3], e_cm;                            /* Eqs. 27, 41: units of c; MeV */
+    double e_ext;                                    /* expectation value of the external terms of Eqs. 24, 26, 36, MeV */
+} lise_ref_observables_ext_t;
 
 typedef struct {
     double energy, e_kin, e_skyrme, e_coul, e_pair;
@@ -81,6 +99,22 @@ int  lise_ref_abm_correct(long n, double dt, const void *y_n, const void *y_nm1,
 /* overwrite the multistep history of one species and mark the context as started (step counter >= 3) */
 int  lise_ref_set_history(lise_ref_ctx *c, int species, const void *y_nm1,
                           const void *f_nm1, const void *f_nm2, const void *f_nm3, const void *e_n);
+/* ---- (f)2: restart (L764-L768), (f)4: boosts, external fields, moving / rotating frame (Eqs. 23-36) ---- */
+/* sets the clock and the total step counter; the multistep start-up state is not touched (after
+ * lise_ref_set_wavefunctions the next three steps use the starter: that is the restart of L764-L768) */
+int  lise_ref_set_time(lise_ref_ctx *c, double time, long step);
+/* Eq. 23: u -> e^{i chi} u, v -> e^{-i chi} v for every state of the species (chi: Nxyz doubles); restarts the multistep method */
+int  lise_ref_boost(lise_ref_ctx *c, int species, const double *chi);
+/* Eq. 24: h_q -> h_q + U0 - (1/2) [Uvec . p + p . Uvec]; u0: Nxyz doubles (MeV), uvec: 3 Nxyz doubles (units of c); NULL = none */
+int  lise_ref_set_external_fields(lise_ref_ctx *c, int species, const double *u0, const double *uvec);
+/* Eqs. 26, 36: h -> h - v_cm . p - omega . (l + s), l = (r - origin) x p; v_cm in units of c, omega in c / fm, origin in fm */
+int  lise_ref_set_frame(lise_ref_ctx *c, const double *v_cm, const double *omega, const double *origin);
+/* Eqs. 37-41 of the current wavefunctions / of externally supplied Table-2 densities and Table-3 potentials */
+int  lise_ref_observables_ext(lise_ref_ctx *c, lise_ref_observables_ext_t *out);
+int  lise_ref_moments_from(lise_ref_ctx *c, const double *dens_n, const double *dens_p,
+                           const double *pot_n, const double *pot_p, lise_ref_observables_ext_t *out);
+/* 1 / g_eff of Eq. 20a for one point (M = hbar^2 / 2 m*, U, mu, E_c in MeV; g0 in MeV fm^3): the pin tests' entry */
+double lise_ref_inv_geff_spherical(double g0, double M, double U, double mu, double e_cut);
 /* pairing constant K of Eq. 21 as the oracle uses it */
 double lise_ref_pairing_K(void);
 

@@ -26,9 +26,27 @@ def build(force=False):
 
 
 class Params(C.Structure):
-    _fields_ = [(n, C.c_double) for n in
-                ("hbar2_2m", "e2", "hbarc", "t0", "t1", "t2", "t3", "x0", "x1", "x2", "x3", "gamma", "W0",
-                 "g0_n", "g0_p")] + [(n, C.c_int) for n in ("coulomb", "pairing_rearrangement", "remove_phase")]
+    _fields_ = ([(n, C.c_double) for n in
+                 ("hbar2_2m", "e2", "hbarc", "t0", "t1", "t2", "t3", "x0", "x1", "x2", "x3", "gamma", "W0",
+                  "g0_n", "g0_p")] + [(n, C.c_int) for n in ("coulomb", "pairing_rearrangement", "remove_phase")]
+                + [(n, C.c_double) for n in ("alpha_pair", "mu_n", "mu_p", "e_cut")]
+                + [(n, C.c_double * 3) for n in ("sea_a", "sea_b", "sea_c")]
+                + [(n, C.c_double * 2) for n in ("sea_cdn", "sea_cdj")]
+                + [(n, C.c_int) for n in ("functional", "pairing_cutoff", "renormalize")])
+
+
+class ObservablesExt(C.Structure):
+    _fields_ = ([(n, C.c_double * 3) for n in ("rcm", "rcm_n", "rcm_p")]
+                + [(n, C.c_double) for n in ("q20", "q30", "q40")] + [("q21", C.c_double * 2), ("q22", C.c_double * 2)]
+                + [(n, C.c_double) for n in ("delta_n", "delta_p", "e_coll")] + [("v_cm", C.c_double * 3)]
+                + [(n, C.c_double) for n in ("e_cm", "e_ext")])
+
+    def as_dict(self):
+        out = {}
+        for n, t in self._fields_:
+            v = getattr(self, n)
+            out[n] = v if isinstance(v, float) else list(v)
+        return out
 
 
 class Observables(C.Structure):
@@ -49,6 +67,9 @@ def lib():
         build()
         _lib = C.CDLL(_SO)
         _lib.lise_ref_pairing_K.restype = C.c_double
+        _lib.lise_ref_inv_geff_spherical.restype = C.c_double
+        _lib.lise_ref_inv_geff_spherical.argtypes = [C.c_double] * 5
+        _lib.lise_ref_set_time.argtypes = [C.c_void_p, C.c_double, C.c_long]
         _lib.lise_ref_abm_predict.argtypes = [C.c_long, C.c_double] + [C.c_void_p] * 9
         _lib.lise_ref_abm_correct.argtypes = [C.c_long, C.c_double] + [C.c_void_p] * 9
     return _lib
@@ -75,6 +96,10 @@ def set_num_threads(n):
 
 def pairing_K():
     return lib().lise_ref_pairing_K()
+
+
+def inv_geff_spherical(g0, M, U, mu, e_cut):
+    return lib().lise_ref_inv_geff_spherical(g0, M, U, mu, e_cut)
 
 
 def abm_predict(dt, y_n, y_nm1, f_n, f_nm1, f_nm2, f_nm3, e_n):
@@ -126,6 +151,37 @@ class RefContext:
     def set_dt(self, dt):
         self.dt = dt
         _chk(lib().lise_ref_set_dt(self._h, C.c_double(dt)), "set_dt")
+
+    def set_time(self, time, step):
+        _chk(lib().lise_ref_set_time(self._h, time, step), "set_time")
+
+    def boost(self, q, chi):
+        a = np.ascontiguousarray(chi, dtype=np.float64)
+        assert a.size == self.nxyz
+        _chk(lib().lise_ref_boost(self._h, q, _p(a)), "boost")
+
+    def set_external_fields(self, q, u0=None, uvec=None):
+        a = None if u0 is None else np.ascontiguousarray(u0, dtype=np.float64)
+        b = None if uvec is None else np.ascontiguousarray(uvec, dtype=np.float64)
+        assert a is None or a.size == self.nxyz
+        assert b is None or b.size == 3 * self.nxyz
+        _chk(lib().lise_ref_set_external_fields(self._h, q, None if a is None else _p(a), None if b is None else _p(b)),
+             "set_external_fields")
+
+    def set_frame(self, v_cm=(0, 0, 0), omega=(0, 0, 0), origin=(0, 0, 0)):
+        arrs = [np.ascontiguousarray(x, dtype=np.float64) for x in (v_cm, omega, origin)]
+        _chk(lib().lise_ref_set_frame(self._h, *[_p(a) for a in arrs]), "set_frame")
+
+    def observables_ext(self):
+        o = ObservablesExt()
+        _chk(lib().lise_ref_observables_ext(self._h, C.byref(o)), "observables_ext")
+        return o.as_dict()
+
+    def moments_from(self, dens_n, dens_p, pot_n, pot_p):
+        arrs = [np.ascontiguousarray(a, dtype=np.float64) for a in (dens_n, dens_p, pot_n, pot_p)]
+        o = ObservablesExt()
+        _chk(lib().lise_ref_moments_from(self._h, *[_p(a) for a in arrs], C.byref(o)), "moments_from")
+        return o.as_dict()
 
     def _blk(self, q, a):
         a = np.ascontiguousarray(a, dtype=np.complex128)

@@ -1195,6 +1195,20 @@ extern "C" int lise_line_operator_tables(int n, double dx, double* tab_host, int
     return LISE_OK;
 }
 
+// host-only: fp64 instruction counts of the generated FFT codelets for a real line of n points (0, 0 if none)
+extern "C" int lise_line_operator_cost(int n, int* inner_ops_host, int* outer_ops_host)
+{
+    if (!inner_ops_host || !outer_ops_host) return LISE_EINVAL;
+    *inner_ops_host = 0; *outer_ops_host = 0;
+    switch (n) {
+#define X(N_) case N_: *inner_ops_host = LineCodelet<N_>::OPS_INNER; *outer_ops_host = LineCodelet<N_>::OPS_OUTER; break;
+    X(4) X(6) X(8) X(10) X(12) X(16) X(20) X(24) X(32) X(40)
+#undef X
+    default: break;
+    }
+    return LISE_OK;
+}
+
 extern "C" const char* lise_line_operator(const lise_ctx* c) { return c ? c->ks.name : "none"; }
 
 extern "C" long lise_launch_count(const lise_ctx* c) { return c ? c->launches : 0; }

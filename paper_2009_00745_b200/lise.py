@@ -32,7 +32,7 @@ EXPORTS = ["lise_default_params", "lise_create", "lise_destroy", "lise_set_param
            "lise_set_dt", "lise_set_chunk", "lise_set_overlap", "lise_set_wavefunctions", "lise_get_wavefunctions",
            "lise_upload_wavefunctions", "lise_download_wavefunctions", "lise_set_reduce_hook",
            "lise_densities", "lise_potentials", "lise_apply_h", "lise_step", "lise_observables",
-           "lise_profile", "lise_profile_read", "lise_measure_fp64_peak", "lise_set_density_group", "lise_line_operator", "lise_line_operator_tables", "lise_launch_count", "lise_device_bytes", "lise_strerror", "lise_last_error"]
+           "lise_profile", "lise_profile_read", "lise_measure_fp64_peak", "lise_set_density_group", "lise_line_operator", "lise_line_operator_cost", "lise_line_operator_tables", "lise_launch_count", "lise_device_bytes", "lise_strerror", "lise_last_error"]
 
 
 REDUCE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_long)
@@ -85,6 +85,7 @@ def load():
     lib.lise_measure_fp64_peak.argtypes = [vp, dp, C.POINTER(dp), C.POINTER(dp)]
     lib.lise_line_operator.argtypes = [vp]; lib.lise_line_operator.restype = C.c_char_p
     lib.lise_set_density_group.argtypes = [vp, ip]
+    lib.lise_line_operator_cost.argtypes = [ip, C.POINTER(ip), C.POINTER(ip)]
     lib.lise_line_operator_tables.argtypes = [ip, dp, C.POINTER(dp), ip, C.POINTER(ip)]
     lib.lise_launch_count.argtypes = [vp]; lib.lise_launch_count.restype = C.c_long
     lib.lise_device_bytes.argtypes = [vp]; lib.lise_device_bytes.restype = C.c_longlong
@@ -110,6 +111,15 @@ def measure_fp64_peak(seconds=1.0, stream=None):
     if rc != 0:
         raise RuntimeError(f"lise_measure_fp64_peak failed ({rc})")
     return tf.value
+
+
+def line_operator_cost(n):
+    """(inner, outer) fp64 instruction counts of the generated FFT code for a real line of n points; host only."""
+    a, b = C.c_int(), C.c_int()
+    rc = load().lise_line_operator_cost(n, C.byref(a), C.byref(b))
+    if rc != 0:
+        raise RuntimeError(f"lise_line_operator_cost failed ({rc})")
+    return a.value, b.value
 
 
 def line_operator_tables(n, dx):
