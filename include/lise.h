@@ -53,7 +53,31 @@ typedef struct {
                                                          * alone decides (it must be the same on every rank of a state-sharded run) */
     int pairing_rearrangement;                          /* 1: include d E_pair / d n in U (reading B8) */
     int remove_phase;                                   /* 1: subtract eta_k = <psi_k|H|psi_k> (Eqs. 80-81)      */
+    /* functional and pairing variants; lise_default_params leaves them off / zero */
+    double alpha_pair;                                  /* Eq. 8: g0(r) = g0 (1 - alpha n(r) / n0), n = n_n + n_p, n0 = 0.16 fm^-3:
+                                                         * 0 volume, 1 surface, 1/2 mixed pairing                              */
+    double mu_n, mu_p, e_cut;                           /* Eq. 20: chemical potentials and energy cutoff E_c (MeV) of the
+                                                         * spherical-cutoff renormalisation (used when pairing_cutoff = 1)   */
+    double sea_a[3], sea_b[3], sea_c[3];                /* Eq. 10: SeaLL1 volume coefficients a_j, b_j, c_j, j = 0..2 (values of
+                                                         * ref. [36], not printed in the paper: supplied by the caller)      */
+    double sea_cdn[2], sea_cdj[2];                      /* SeaLL1: C_t^{n Delta n} and C_t^{nabla J}, t = 0, 1                */
+    int functional;                                     /* 0: Skyrme functional (Eq. 9); 1: SeaLL1 (Eqs. 10, 15; m* = m)     */
+    int pairing_cutoff;                                 /* 0: lattice cutoff, Eq. 21; 1: spherical cutoff, Eq. 20 (no pairing
+                                                         * rearrangement term then: DESIGN.md reading B30)                   */
+    int renormalize;                                    /* 1: every qpwf is normalised at the end of each step */
 } lise_params;
+
+/* Observables of PAPER.md Eqs. 37-41 (L304-L335) of the current wavefunctions y_n, and the energy of the external
+ * terms.  Coordinates are x_i = i dx (Eq. 43); the multipoles are taken about the total centre of mass (L367). */
+typedef struct {
+    double rcm[3], rcm_n[3], rcm_p[3];                  /* Eq. 37: centre of mass of nucleons, neutrons, protons, fm            */
+    double q20, q30, q40, q21[2], q22[2];               /* Eq. 38 b-e of the total density: 2z^2-x^2-y^2, z(2z^2-3x^2-3y^2),
+                                                         * 35z^4-30z^2r^2+3r^4, (x+iy)z and (x+iy)^2 as (re, im)               */
+    double delta_n, delta_p;                            /* Eq. 39: density-weighted average of |Delta_q|, MeV                   */
+    double e_coll;                                      /* Eq. 40 read as sum_q int (hbar^2/2m) j_q^2 / n_q (B31), MeV */
+    double v_cm[3], e_cm;                               /* Eqs. 27, 41: hbar int j / (m A) in units of c; (1/2) m A v_cm^2, MeV  */
+    double e_ext;                                       /* expectation value of the external terms (Eqs. 24, 26, 36), MeV       */
+} lise_observables_ext_t;
 
 /* Observables of the current wavefunctions y_n (E(t), Z(t), N(t)). */
 typedef struct {
@@ -136,6 +160,26 @@ int lise_set_reduce_hook(lise_ctx *ctx, lise_reduce_fn fn, void *user);
 
 /* Energy, particle numbers, norm / orthonormality defects of the current wavefunctions. Synchronises. */
 int lise_observables(lise_ctx *ctx, lise_observables_t *host_out);
+/* Eqs. 37-41 as grid reductions of the Table-2 / Table-3 fields of the current wavefunctions.  Synchronises. */
+int lise_observables_ext(lise_ctx *ctx, lise_observables_ext_t *host_out);
+
+/* Checkpoint / restart: a checkpoint is lise_download_wavefunctions (only the latest wavefunctions
+ * are saved) plus the clock; a restart is lise_create + lise_upload_wavefunctions (keep_history = 0: the next three
+ * steps go through the series expansion) + lise_set_time, which sets the clock (fm/c) and the step counter that
+ * lise_observables reports, without touching the multistep start-up state. */
+int lise_set_time(lise_ctx *ctx, double time, long step);
+
+/* Boost (Eq. 23): u -> e^{i chi} u, v -> e^{-i chi} v for every state of the species; chi_dev: Nxyz doubles (DEVICE).
+ * Re-accumulates the densities and restarts the multistep method (the next three steps use the starter). */
+int lise_boost(lise_ctx *ctx, int species, const double *chi_dev);
+/* External fields (Eq. 24): h_q -> h_q + U0 - (1/2) [Uvec . p + p . Uvec].  u0_dev: Nxyz doubles (MeV), uvec_dev:
+ * 3 Nxyz doubles, component-major, in units of c; DEVICE pointers, copied into the context; NULL removes the field. */
+int lise_set_external_fields(lise_ctx *ctx, int species, const double *u0_dev, const double *uvec_dev);
+/* Moving and rotating frame (Eqs. 26, 36): h -> h - v_cm . p - omega . (l + s) for both species, l = (r - origin) x p;
+ * v_cm_host in units of c, omega_host in c / fm, origin_host in fm (HOST pointers to 3 doubles; NULL = zero). */
+int lise_set_frame(lise_ctx *ctx, const double *v_cm_host, const double *omega_host, const double *origin_host);
+/* lise_potentials returns the fields that enter H: U includes U0, A includes -(hbar c / 2) (Uvec + v_cm + omega x r),
+ * S includes -(hbar c / 2) omega. */
 
 /* Per-kernel-class device timing with CUDA events on the context's stream (for bench.py's roofline).
  * lise_profile(ctx, 1) starts recording an event pair around every launch of the per-state kernels

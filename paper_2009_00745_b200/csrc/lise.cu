@@ -66,6 +66,10 @@ struct lise_ctx {
     KernSet ks;
     int have[2], pot_valid;
     long step; double time;
+    long since;                             // steps since the multistep method was (re)started: < 3 -> starter
+    double *uext[2], *vext[2];              // external fields of Eq. 24 in use (NULL = none) ...
+    double *uext_buf[2], *vext_buf[2];      // ... and the context's buffers that hold them
+    double* mbuf; double* nrm;              // reduction scratch of the Eq. 37-41 observables; state norms (renormalisation)
     long launches; long long bytes;
     std::vector<void*>* allocs;
     // optional per-kernel-class timing with CUDA events on the context's stream (lise_profile)
@@ -219,16 +223,23 @@ static void set_physconst(lise_ctx* c)
     PhysConst& k = c->pc;
     k.h2m = p.hbar2_2m; k.e2 = p.e2; k.hbarc = p.hbarc; k.gamma = p.gamma; k.a = c->L.dx;
     k.Kc = 2.442749607806335;
-    // couplings of Eq. 9 from the Skyrme parameters (standard relations, DESIGN.md A.0)
-    k.Cn[0] = 3.0 * p.t0 / 8.0;                       k.Cn[1] = -(p.t0 / 4.0) * (0.5 + p.x0);
-    k.Cg[0] = p.t3 / 16.0;                            k.Cg[1] = -(p.t3 / 24.0) * (0.5 + p.x3);
-    k.Cd[0] = -9.0 * p.t1 / 64.0 + (p.t2 / 16.0) * (1.25 + p.x2);
-    k.Cd[1] = (3.0 * p.t1 / 32.0) * (0.5 + p.x1) + (p.t2 / 32.0) * (0.5 + p.x2);
-    k.Ct[0] = 3.0 * p.t1 / 16.0 + (p.t2 / 4.0) * (1.25 + p.x2);
-    k.Ct[1] = -(p.t1 / 8.0) * (0.5 + p.x1) + (p.t2 / 8.0) * (0.5 + p.x2);
-    k.CJ[0] = -3.0 * p.W0 / 4.0;                      k.CJ[1] = -p.W0 / 4.0;
+    if (p.functional == 1) {
+        // SeaLL1 (Eq. 10): volume term by its own coefficients, gradient and spin-orbit couplings supplied, m* = m
+        for (int t = 0; t < 2; ++t) { k.Cn[t] = k.Cg[t] = k.Ct[t] = 0.0; k.Cd[t] = p.sea_cdn[t]; k.CJ[t] = p.sea_cdj[t]; }
+    } else {
+        // couplings of Eq. 9 from the Skyrme parameters (standard relations, DESIGN.md A.0)
+        k.Cn[0] = 3.0 * p.t0 / 8.0;                       k.Cn[1] = -(p.t0 / 4.0) * (0.5 + p.x0);
+        k.Cg[0] = p.t3 / 16.0;                            k.Cg[1] = -(p.t3 / 24.0) * (0.5 + p.x3);
+        k.Cd[0] = -9.0 * p.t1 / 64.0 + (p.t2 / 16.0) * (1.25 + p.x2);
+        k.Cd[1] = (3.0 * p.t1 / 32.0) * (0.5 + p.x1) + (p.t2 / 32.0) * (0.5 + p.x2);
+        k.Ct[0] = 3.0 * p.t1 / 16.0 + (p.t2 / 4.0) * (1.25 + p.x2);
+        k.Ct[1] = -(p.t1 / 8.0) * (0.5 + p.x1) + (p.t2 / 8.0) * (0.5 + p.x2);
+        k.CJ[0] = -3.0 * p.W0 / 4.0;                      k.CJ[1] = -p.W0 / 4.0;
+    }
     k.g0[0] = p.g0_n; k.g0[1] = p.g0_p;
-    k.coulomb = p.coulomb; k.rearr = p.pairing_rearrangement;
+    k.alpha = p.alpha_pair; k.mu[0] = p.mu_n; k.mu[1] = p.mu_p; k.ecut = p.e_cut;
+    for (int j = 0; j < 3; ++j) { k.sa[j] = p.sea_a[j]; k.sb[j] = p.sea_b[j]; k.sc[j] = p.sea_c[j]; }
+    k.coulomb = p.coulomb; k.rearr = p.pairing_rearrangement; k.functional = p.functional; k.cutoff = p.pairing_cutoff;
 }
 
 extern "C" int lise_default_params(lise_params* p)
@@ -240,6 +251,10 @@ extern "C" int lise_default_params(lise_params* p)
     p->gamma = 1.0 / 6.0; p->W0 = 123.0;
     p->g0_n = -250.0; p->g0_p = -250.0;
     p->coulomb = 1; p->pairing_rearrangement = 1; p->remove_phase = 1;
+    p->alpha_pair = 0.0; p->mu_n = p->mu_p = 0.0; p->e_cut = 0.0;
+    for (int j = 0; j < 3; ++j) p->sea_a[j] = p->sea_b[j] = p->sea_c[j] = 0.0;
+    p->sea_cdn[0] = p->sea_cdn[1] = p->sea_cdj[0] = p->sea_cdj[1] = 0.0;
+    p->functional = 0; p->pairing_cutoff = 0; p->renormalize = 0;
     return LISE_OK;
 }
 
@@ -363,7 +378,7 @@ static KernSet make_v6_set()
     return k;
 }
 #define LISE_FFT_SHAPES(X) \
-    X(8, 8, 8) X(12, 12, 12) X(16, 16, 16) X(20, 20, 20) X(24, 24, 24) X(32, 32, 32) X(12, 8, 16) X(16, 12, 8)
+    X(8, 8, 8) X(12, 12, 12) X(16, 16, 16) X(20, 20, 20) X(24, 24, 24) X(32, 32, 32) X(12, 8, 16) X(16, 12, 8) X(12, 12, 16)
 
 // The DMMA plane kernels are instantiated for these lattices (nx, ny, nz): every lattice of BASELINE.json's
 // configs, the paper's 24^2 x 48, and two small non-cubic test shapes; every edge a multiple of 4 and the
@@ -559,7 +574,9 @@ static int compute_potentials(lise_ctx* c)
     const int nx = c->L.nxyz;
     if (c->pc.coulomb) TRY(coulomb(c, c->acc[1] + (size_t)ACC_N * nx));
     k_grid_deriv<<<dim3(nblk(nx, 128), c->njobs1), 128, 0, c->stream>>>(c->L, c->jobs1, c->ctab[0], c->ctab[1], c->ctab[2]); CKL();
-    k_potentials<<<nblk(nx, 128), 128, 0, c->stream>>>(c->L, c->pc, c->acc[0], c->acc[1], c->gtmp, c->phi,
+    ExtFields ext;
+    for (int q = 0; q < 2; ++q) { ext.u0[q] = c->uext[q]; ext.uvec[q] = c->vext[q]; }
+    k_potentials<<<nblk(nx, 128), 128, 0, c->stream>>>(c->L, c->pc, ext, c->acc[0], c->acc[1], c->gtmp, c->phi,
                                                         c->dens[0], c->dens[1], c->pot[0], c->pot[1], c->geff[0], c->geff[1]); CKL();
     k_grid_deriv<<<dim3(nblk(nx, 128), c->njobs2), 128, 0, c->stream>>>(c->L, c->jobs2, c->ctab[0], c->ctab[1], c->ctab[2]); CKL();
     k_uloc<<<nblk(nx, 128), 128, 0, c->stream>>>(nx, c->pot[0], c->pot[1]); CKL();
@@ -581,6 +598,18 @@ static int ensure_potentials(lise_ctx* c)
     if (c->pot_valid) return LISE_OK;
     TRY(grid_phase(c, 1));
     c->pot_valid = 1;
+    return LISE_OK;
+}
+
+// L637: psi_k <- psi_k / sqrt(<psi_k|psi_k>) for every state of slot `r` of both species (optional, lise_params.renormalize)
+static int renormalize_slot(lise_ctx* c, int r)
+{
+    const size_t slen = (size_t)4 * c->L.nxyz;
+    for (int q = 0; q < 2; ++q) {
+        if (c->nwf[q] == 0) continue;
+        k_state_norms<<<c->nwf[q], 256, 0, c->stream>>>(S(c, q, r), slen, c->L.dV, c->nrm); CKL();
+        k_state_scale<<<dim3(nblk(slen, 256), c->nwf[q]), 256, 0, c->stream>>>(S(c, q, r), slen, c->nrm); CKL();
+    }
     return LISE_OK;
 }
 
@@ -625,6 +654,7 @@ static int abm_step(lise_ctx* c)
                 if (pipe) { CK(cudaEventRecord(c->ev_h[wb], c->stream)); CK(cudaStreamWaitEvent(c->stream2, c->ev_h[wb], 0)); }
                 if (phase == 1) TRY(launch_update<1>(c, u, su)); else TRY(launch_update<2>(c, u, su));
                 if (pipe) CK(cudaEventRecord(c->ev_u[wb], c->stream2));
+                if (phase == 2 && c->par.renormalize) continue;    // densities of y_{n+1} follow the rescaling below
                 if (c->ks.v5) {
                     if (pend_q >= 0 && (pend_q != q || pend_chunks >= c->dgroup)) TRY(flush_dens(i - 1));
                     if (pend_q < 0) { pend_q = q; pend_off = off; }
@@ -634,6 +664,14 @@ static int abm_step(lise_ctx* c)
                 }
             }
         TRY(flush_dens(i - 1));
+        if (phase == 2 && c->par.renormalize) {
+            if (pipe) for (int b = 0; b < 2; ++b) CK(cudaStreamWaitEvent(c->stream, c->ev_u[b], 0));   // all updates done
+            TRY(renormalize_slot(c, RB));
+            for (int q = 0; q < 2; ++q) {
+                TRY(zero_partials(c, q));              // (the generic update kernels already added y/z parts of the unscaled state)
+                if (c->nwf[q] > 0) TRY(dens_accumulate(c, q, S(c, q, RB)));
+            }
+        }
         if (phase == 1) TRY(grid_phase(c, 1));     // potentials of the modifier m
     }
     // y_{n+1} sits in B: A <-> B; f history shifts
@@ -678,6 +716,7 @@ static int starter_step(lise_ctx* c)
     for (int q = 0; q < 2; ++q) { k_average<<<nblk(nacc, 256), 256, 0, c->stream>>>(c->acc[q], c->acc0[q], nacc); CKL(); }
     TRY(compute_potentials(c));                     // H_cor
     TRY(taylor4_all(c, 0));                         // y_{n+1} -> F
+    if (c->par.renormalize) TRY(renormalize_slot(c, RF));
     for (int q = 0; q < 2; ++q) {
         TRY(zero_partials(c, q));
         TRY(dens_accumulate(c, q, S(c, q, RF)));
@@ -867,6 +906,8 @@ static int ctx_init(lise_ctx* c)
     if (c->par.coulomb) TRY(alloc_coulomb(c));
     c->eblocks = 64;
     DM(c->ebuf, c->eblocks * 6);
+    DM(c->mbuf, c->eblocks * 16);
+    DM(c->nrm, nmax > 0 ? nmax : 1);
     DM(c->ovl, (size_t)(nmax > 0 ? nmax : 1) * 4);
     return LISE_OK;
 }
@@ -943,7 +984,7 @@ extern "C" int lise_set_stream(lise_ctx* c, void* s)
 extern "C" int lise_set_dt(lise_ctx* c, double dt)
 {
     if (!c) return LISE_EINVAL;
-    c->dt = dt; c->step = 0;
+    c->dt = dt; c->step = 0; c->since = 0;
     return LISE_OK;
 }
 
@@ -976,7 +1017,7 @@ extern "C" int lise_set_wavefunctions(lise_ctx* c, int q, const void* psi_dev)
     if (c->nwf[q] > 0) CK(cudaMemcpyAsync(S(c, q, RA), psi_dev, bytes, cudaMemcpyDeviceToDevice, c->stream));
     TRY(zero_partials(c, q));
     if (c->nwf[q] > 0) TRY(dens_accumulate(c, q, S(c, q, RA)));
-    c->have[q] = 1; c->pot_valid = 0; c->step = 0; c->time = 0.0;
+    c->have[q] = 1; c->pot_valid = 0; c->step = 0; c->since = 0; c->time = 0.0;
     return LISE_OK;
 }
 
@@ -998,7 +1039,7 @@ extern "C" int lise_upload_wavefunctions(lise_ctx* c, int q, const void* psi_hos
     TRY(zero_partials(c, q));
     if (c->nwf[q] > 0) TRY(dens_accumulate(c, q, S(c, q, RA)));
     c->have[q] = 1; c->pot_valid = 0;
-    if (!keep_history) { c->step = 0; c->time = 0.0; }
+    if (!keep_history) { c->step = 0; c->since = 0; c->time = 0.0; }
     return LISE_OK;
 }
 
@@ -1072,8 +1113,8 @@ static int step_impl(lise_ctx* c, int nsteps)
     }
     int rc = LISE_OK;
     for (int s = 0; s < nsteps && rc == LISE_OK; ++s) {
-        rc = (c->step < 3) ? starter_step(c) : abm_step(c);
-        if (rc == LISE_OK) { c->step += 1; c->time += c->dt; }
+        rc = (c->since < 3) ? starter_step(c) : abm_step(c);
+        if (rc == LISE_OK) { c->step += 1; c->since += 1; c->time += c->dt; }
     }
     if (fork) {
         c->stream = user; c->user_stream_valid = 0;
@@ -1092,7 +1133,7 @@ static int observables_impl(lise_ctx* c, lise_observables_t* o)
     if (!c || !o) return LISE_EINVAL;
     TRY(need_both(c));
     TRY(ensure_potentials(c));
-    k_energy<<<c->eblocks, 256, 0, c->stream>>>(c->L, c->pc, c->dens[0], c->dens[1], c->gtmp, c->phi, c->geff[0], c->geff[1], c->ebuf); CKL();
+    k_energy<<<c->eblocks, 256, 0, c->stream>>>(c->L, c->pc, c->acc[0], c->acc[1], c->gtmp, c->phi, c->geff[0], c->geff[1], c->ebuf); CKL();
     std::vector<double> eb(c->eblocks * 6);
     CK(cudaMemcpyAsync(eb.data(), c->ebuf, sizeof(double) * eb.size(), cudaMemcpyDeviceToHost, c->stream));
     double nd = 0.0, od = 0.0;
@@ -1127,6 +1168,97 @@ static int observables_impl(lise_ctx* c, lise_observables_t* o)
 extern "C" int lise_observables(lise_ctx* c, lise_observables_t* o)
 {
     return guarded([&] { return observables_impl(c, o); });
+}
+
+extern "C" int lise_set_time(lise_ctx* c, double time, long step)
+{
+    if (!c || step < 0) return LISE_EINVAL;
+    c->time = time; c->step = step;
+    return LISE_OK;
+}
+
+extern "C" int lise_boost(lise_ctx* c, int q, const double* chi_dev)
+{
+    if (!c || q < 0 || q > 1 || !chi_dev) return LISE_EINVAL;
+    if (!c->have[q]) { snprintf(c->err, sizeof(c->err), "wavefunctions of species %d not set", q); return LISE_ESTATE; }
+    if (c->nwf[q] > 0) {
+        k_boost<<<dim3(nblk(c->L.nxyz, 128), 4, c->nwf[q]), 128, 0, c->stream>>>(S(c, q, RA), chi_dev, c->L.nxyz); CKL();
+    }
+    TRY(zero_partials(c, q));
+    if (c->nwf[q] > 0) TRY(dens_accumulate(c, q, S(c, q, RA)));
+    c->pot_valid = 0; c->since = 0;
+    return LISE_OK;
+}
+
+extern "C" int lise_set_external_fields(lise_ctx* c, int q, const double* u0_dev, const double* uvec_dev)
+{
+    if (!c || q < 0 || q > 1) return LISE_EINVAL;
+    const size_t nx = c->L.nxyz;
+    // the buffers are allocated once and kept; a NULL argument switches the field off
+    if (u0_dev) {
+        if (!c->uext_buf[q]) DM(c->uext_buf[q], nx);
+        CK(cudaMemcpyAsync(c->uext_buf[q], u0_dev, sizeof(double) * nx, cudaMemcpyDeviceToDevice, c->stream));
+    }
+    if (uvec_dev) {
+        if (!c->vext_buf[q]) DM(c->vext_buf[q], 3 * nx);
+        CK(cudaMemcpyAsync(c->vext_buf[q], uvec_dev, sizeof(double) * 3 * nx, cudaMemcpyDeviceToDevice, c->stream));
+    }
+    c->uext[q] = u0_dev ? c->uext_buf[q] : nullptr;
+    c->vext[q] = uvec_dev ? c->vext_buf[q] : nullptr;
+    c->pot_valid = 0;
+    return LISE_OK;
+}
+
+extern "C" int lise_set_frame(lise_ctx* c, const double* v_cm, const double* omega, const double* origin)
+{
+    if (!c) return LISE_EINVAL;
+    for (int i = 0; i < 3; ++i) {
+        c->pc.vcm[i] = v_cm ? v_cm[i] : 0.0; c->pc.omega[i] = omega ? omega[i] : 0.0; c->pc.origin[i] = origin ? origin[i] : 0.0;
+    }
+    c->pot_valid = 0;
+    return LISE_OK;
+}
+
+static int observables_ext_impl(lise_ctx* c, lise_observables_ext_t* o)
+{
+    if (!c || !o) return LISE_EINVAL;
+    TRY(need_both(c));
+    TRY(ensure_potentials(c));
+    ExtFields ext;
+    for (int q = 0; q < 2; ++q) { ext.u0[q] = c->uext[q]; ext.uvec[q] = c->vext[q]; }
+    const int nb = c->eblocks;
+    k_moments1<<<nb, 256, 0, c->stream>>>(c->L, c->pc, ext, c->dens[0], c->dens[1], c->pot[0], c->pot[1], c->mbuf); CKL();
+    std::vector<double> hb((size_t)nb * 16);
+    CK(cudaMemcpyAsync(hb.data(), c->mbuf, sizeof(double) * hb.size(), cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    double m[16];
+    for (int k = 0; k < 16; ++k) { m[k] = 0.0; for (int b = 0; b < nb; ++b) m[k] += hb[(size_t)b * 16 + k]; }
+    const double Nn = m[0], Np = m[1], A = Nn + Np;
+    for (int i = 0; i < 3; ++i) {
+        o->rcm_n[i] = Nn > 0.0 ? m[2 + i] / Nn : 0.0;
+        o->rcm_p[i] = Np > 0.0 ? m[5 + i] / Np : 0.0;
+        o->rcm[i] = A > 0.0 ? (m[2 + i] + m[5 + i]) / A : 0.0;
+    }
+    o->delta_n = Nn > 0.0 ? m[11] / Nn : 0.0;
+    o->delta_p = Np > 0.0 ? m[12] / Np : 0.0;
+    o->e_coll = m[13];
+    o->e_ext = m[14];
+    // Eq. 27: v_cm = hbar int j d^3r / (m A); hbar / m = 2 (hbar^2 / 2m) / (hbar c) in units of c.  Eq. 41: (1/2) m A v_cm^2
+    double j2 = 0.0;
+    for (int i = 0; i < 3; ++i) { o->v_cm[i] = A > 0.0 ? 2.0 * c->par.hbar2_2m / c->par.hbarc * m[8 + i] / A : 0.0; j2 += m[8 + i] * m[8 + i]; }
+    o->e_cm = A > 0.0 ? c->par.hbar2_2m * j2 / A : 0.0;
+    k_moments2<<<nb, 256, 0, c->stream>>>(c->L, c->dens[0], c->dens[1], o->rcm[0], o->rcm[1], o->rcm[2], c->mbuf); CKL();
+    CK(cudaMemcpyAsync(hb.data(), c->mbuf, sizeof(double) * (size_t)nb * 8, cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    double qm[8];
+    for (int k = 0; k < 8; ++k) { qm[k] = 0.0; for (int b = 0; b < nb; ++b) qm[k] += hb[(size_t)b * 8 + k]; }
+    o->q20 = qm[0]; o->q30 = qm[1]; o->q40 = qm[2];
+    o->q21[0] = qm[3]; o->q21[1] = qm[4]; o->q22[0] = qm[5]; o->q22[1] = qm[6];
+    return LISE_OK;
+}
+extern "C" int lise_observables_ext(lise_ctx* c, lise_observables_ext_t* o)
+{
+    return guarded([&] { return observables_ext_impl(c, o); });
 }
 
 extern "C" int lise_profile(lise_ctx* c, int enable)

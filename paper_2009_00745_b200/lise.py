@@ -14,9 +14,27 @@ _lib = None
 
 
 class Params(C.Structure):
-    _fields_ = [(n, C.c_double) for n in
-                ("hbar2_2m", "e2", "hbarc", "t0", "t1", "t2", "t3", "x0", "x1", "x2", "x3", "gamma", "W0",
-                 "g0_n", "g0_p")] + [(n, C.c_int) for n in ("coulomb", "pairing_rearrangement", "remove_phase")]
+    _fields_ = ([(n, C.c_double) for n in
+                 ("hbar2_2m", "e2", "hbarc", "t0", "t1", "t2", "t3", "x0", "x1", "x2", "x3", "gamma", "W0",
+                  "g0_n", "g0_p")] + [(n, C.c_int) for n in ("coulomb", "pairing_rearrangement", "remove_phase")]
+                + [(n, C.c_double) for n in ("alpha_pair", "mu_n", "mu_p", "e_cut")]
+                + [(n, C.c_double * 3) for n in ("sea_a", "sea_b", "sea_c")]
+                + [(n, C.c_double * 2) for n in ("sea_cdn", "sea_cdj")]
+                + [(n, C.c_int) for n in ("functional", "pairing_cutoff", "renormalize")])
+
+
+class ObservablesExt(C.Structure):
+    _fields_ = ([(n, C.c_double * 3) for n in ("rcm", "rcm_n", "rcm_p")]
+                + [(n, C.c_double) for n in ("q20", "q30", "q40")] + [("q21", C.c_double * 2), ("q22", C.c_double * 2)]
+                + [(n, C.c_double) for n in ("delta_n", "delta_p", "e_coll")] + [("v_cm", C.c_double * 3)]
+                + [(n, C.c_double) for n in ("e_cm", "e_ext")])
+
+    def as_dict(self):
+        out = {}
+        for n, _ in self._fields_:
+            v = getattr(self, n)
+            out[n] = v if isinstance(v, float) else list(v)
+        return out
 
 
 class Observables(C.Structure):
@@ -31,7 +49,8 @@ class Observables(C.Structure):
 EXPORTS = ["lise_default_params", "lise_create", "lise_destroy", "lise_set_params", "lise_set_stream",
            "lise_set_dt", "lise_set_chunk", "lise_set_overlap", "lise_set_wavefunctions", "lise_get_wavefunctions",
            "lise_upload_wavefunctions", "lise_download_wavefunctions", "lise_set_reduce_hook",
-           "lise_densities", "lise_potentials", "lise_apply_h", "lise_step", "lise_observables",
+           "lise_densities", "lise_potentials", "lise_apply_h", "lise_step", "lise_observables", "lise_observables_ext",
+           "lise_set_time", "lise_boost", "lise_set_external_fields", "lise_set_frame",
            "lise_profile", "lise_profile_read", "lise_measure_fp64_peak", "lise_set_density_group", "lise_line_operator", "lise_line_operator_cost", "lise_line_operator_tables", "lise_launch_count", "lise_device_bytes", "lise_strerror", "lise_last_error"]
 
 
@@ -80,6 +99,11 @@ def load():
     lib.lise_apply_h.argtypes = [vp, ip, vp, vp, ip]
     lib.lise_step.argtypes = [vp, ip]
     lib.lise_observables.argtypes = [vp, C.POINTER(Observables)]
+    lib.lise_observables_ext.argtypes = [vp, C.POINTER(ObservablesExt)]
+    lib.lise_set_time.argtypes = [vp, dp, C.c_long]
+    lib.lise_boost.argtypes = [vp, ip, vp]
+    lib.lise_set_external_fields.argtypes = [vp, ip, vp, vp]
+    lib.lise_set_frame.argtypes = [vp, C.POINTER(dp), C.POINTER(dp), C.POINTER(dp)]
     lib.lise_profile.argtypes = [vp, ip]
     lib.lise_profile_read.argtypes = [vp, C.POINTER(dp), C.POINTER(C.c_long)]
     lib.lise_measure_fp64_peak.argtypes = [vp, dp, C.POINTER(dp), C.POINTER(dp)]
@@ -301,6 +325,26 @@ class Lise:
         self._chk(self.lib.lise_observables(self._h, C.byref(o)), "lise_observables")
         return o.as_dict()
 
+    def observables_ext(self):
+        o = ObservablesExt()
+        self._chk(self.lib.lise_observables_ext(self._h, C.byref(o)), "lise_observables_ext")
+        return o.as_dict()
+
+    def set_time(self, time, step):
+        self._chk(self.lib.lise_set_time(self._h, time, step), "lise_set_time")
+
+    def boost(self, q, chi):
+        self._chk(self.lib.lise_boost(self._h, q, self._dev(chi, torch.float64, self.nxyz)), "lise_boost")
+
+    def set_external_fields(self, q, u0=None, uvec=None):
+        a = C.c_void_p() if u0 is None else self._dev(u0, torch.float64, self.nxyz)
+        b = C.c_void_p() if uvec is None else self._dev(uvec, torch.float64, 3 * self.nxyz)
+        self._chk(self.lib.lise_set_external_fields(self._h, q, a, b), "lise_set_external_fields")
+
+    def set_frame(self, v_cm=(0.0, 0.0, 0.0), omega=(0.0, 0.0, 0.0), origin=(0.0, 0.0, 0.0)):
+        arrs = [(C.c_double * 3)(*[float(x) for x in v]) for v in (v_cm, omega, origin)]
+        self._chk(self.lib.lise_set_frame(self._h, *arrs), "lise_set_frame")
+
     PROFILE_CLASSES = ("happly_yz", "happly_xz", "update", "dens_x", "grid", "dens_yz")
 
     def profile(self, enable=True):
@@ -332,7 +376,7 @@ def _on_device(method):
     return wrapper
 
 
-for _name in ("close", "set_params", "set_stream", "set_density_group", "set_dt", "set_chunk", "set_overlap",
+for _name in ("observables_ext", "boost", "set_external_fields", "close", "set_params", "set_stream", "set_density_group", "set_dt", "set_chunk", "set_overlap",
               "set_wavefunctions", "get_wavefunctions", "upload_wavefunctions", "download_wavefunctions",
               "set_reduce_hook", "densities", "potentials", "apply_h", "step", "observables", "profile", "profile_read"):
     setattr(Lise, _name, _on_device(getattr(Lise, _name)))
