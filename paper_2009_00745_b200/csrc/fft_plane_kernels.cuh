@@ -141,6 +141,17 @@ constexpr int tmem_cols(int warps, int n)
     return c;
 }
 
+// ---- TMA (cp.async.bulk.tensor): one thread loads a whole [rows][128 bytes] plane tile, SWIZZLE_128B, completing on an mbarrier ----
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes)
+{
+    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n\t}" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void tma_load_tile(unsigned dst, const CUtensorMap* tm, unsigned long long* bar, int c0, int c1, int c2, int c3)
+{
+    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+                 ::"r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar)) : "memory");
+}
+
 struct LaneRole {
     int j, s, p;            // line within the task (0..7), spin component (0 up, 1 down), part (0 re, 1 im)
     unsigned pm, sm;        // sign-bit masks: sp = -1 for the imaginary part, ss = -1 for the down component (else +1)
@@ -266,7 +277,7 @@ struct YZGeom {
 };
 
 template <int NY, int NZ, int NCOMP, int MAXR, bool PAIRING>
-__global__ void __maxnreg__(MAXR) k6_happly_yz(HArgs a)
+__global__ void __maxnreg__(MAXR) k6_happly_yz(const __grid_constant__ HArgs a)
 {
     static_assert(!PAIRING || NCOMP == 4, "the pairing block needs the whole state in the unit");
     typedef YZGeom<NY, NZ, NCOMP> G;
@@ -287,22 +298,23 @@ __global__ void __maxnreg__(MAXR) k6_happly_yz(HArgs a)
     const double* pot = a.pot;
     const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);   // warp-uniform for the compiler: the role branch below does not diverge
     if (threadIdx.x == 0) {
-        mbar_init(barF, NTHR); mbar_init(barF + 1, NTHR);
+        mbar_init(barF, 1); mbar_init(barF + 1, 1);               // "unit landed": one arrival (expect_tx) + the TMA's bytes
         mbar_init(barE, NTHR); mbar_init(barE + 1, NTHR);
         mbar_init(barZ, G::NWZ * 32);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     const unsigned tbase = tmem_alloc<G::TCOLS>(&s_tmem, warp);     // includes a CTA-wide barrier
     const unsigned tr = tbase + ((unsigned)(warp & 3) << 21) + (unsigned)(warp >> 2) * (2 * NMAX);
     const int nunits = a.ns * UPS;
+    // one thread stages a unit: NCOMP x NT tensor-map tile copies ([NY rows][128 bytes], hardware-swizzled)
     auto issue = [&](int u, int buf) {
-        const int st = u / UPS, pg = u - st * UPS;
-        const cplx* Xs = a.X + ((size_t)st * 4 + pg * NCOMP) * nxyz + gbase;
-        cplx* dst = phi + buf * NCOMP * SZ;
-        for (int i = threadIdx.x; i < NCOMP * NPTS; i += NTHR) {
-            const int c = i / NPTS, p = i - c * NPTS, y = p / NZ, z = p - y * NZ;
-            cp_async16(dst + c * SZ + PL::idx(y, z), Xs + (size_t)c * nxyz + p);
-        }
-        mbar_arrive_cp_async(barF + buf);
+        if (threadIdx.x != 0) return;
+        mbar_expect_tx(barF + buf, NCOMP * PL::NT * NY * 128);
+#pragma unroll
+        for (int c = 0; c < NCOMP; ++c)
+#pragma unroll
+            for (int t = 0; t < PL::NT; ++t)
+                tma_load_tile(s_phi + ((buf * NCOMP + c) * SZ + t * TS) * 16, &a.tmX, barF + buf, 16 * t, 0, (int)blockIdx.x, u * NCOMP + c);
     };
     int u = blockIdx.y;
     if (u < nunits) issue(u, 0);
@@ -401,7 +413,7 @@ struct XZGeom {
 };
 
 template <int NX, int NZ, int MAXR>
-__global__ void __maxnreg__(MAXR) k6_happly_xz(HArgs a)
+__global__ void __maxnreg__(MAXR) k6_happly_xz(const __grid_constant__ HArgs a)
 {
     typedef XZGeom<NX, NZ> G;
     typedef typename G::PL PL;
@@ -421,20 +433,22 @@ __global__ void __maxnreg__(MAXR) k6_happly_xz(HArgs a)
     const double* pot = a.pot;
     const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
     if (threadIdx.x == 0) {
-        mbar_init(barF, NTHR); mbar_init(barF + 1, NTHR);
+        mbar_init(barF, 1); mbar_init(barF + 1, 1);
         mbar_init(barE, NTHR); mbar_init(barE + 1, NTHR);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     const unsigned tbase = tmem_alloc<G::TCOLS>(&s_tmem, warp);
     const unsigned tr = tbase + ((unsigned)(warp & 3) << 21) + (unsigned)(warp >> 2) * (2 * NX);
     const int nunits = a.ns;
+    // one thread stages a unit: 4 x NT tensor-map tile copies ([NX rows at stride ny nz][128 bytes], hardware-swizzled)
     auto issue = [&](int u, int buf) {
-        const size_t go = (size_t)u * 4 * nxyz + gb;
-        cplx* dst = phi + buf * 4 * SZ;
-        for (int i = threadIdx.x; i < 4 * NPTS; i += NTHR) {
-            const int c = i / NPTS, p = i - c * NPTS, x = p / NZ, z = p - x * NZ;
-            cp_async16(dst + c * SZ + PL::idx(x, z), a.X + go + (size_t)c * nxyz + (size_t)x * gs + z);
-        }
-        mbar_arrive_cp_async(barF + buf);
+        if (threadIdx.x != 0) return;
+        mbar_expect_tx(barF + buf, 4 * PL::NT * NX * 128);
+#pragma unroll
+        for (int c = 0; c < 4; ++c)
+#pragma unroll
+            for (int t = 0; t < PL::NT; ++t)
+                tma_load_tile(s_phi + ((buf * 4 + c) * SZ + t * TS) * 16, &a.tmX, barF + buf, 16 * t, (int)blockIdx.x, 0, u * 4 + c);
     };
     auto flush_eta = [&](int uprev, int it_prev) {               // thread 0: fixed-order sum of the warps' partials
         double s = 0.0;

@@ -30,6 +30,7 @@ struct KernSet {
     size_t smem_h[2], smem_u, smem_d, smem_dyz;   // dynamic shared memory, bytes (0 = filled by ctx_init for the generic path)
     int ups_xz;                            // eta partial sums per state = ups_xz * ny
     int cps_h[2];                          // resident CTAs per SM of the two H-apply kernels (state groups = G * cps)
+    int tma_h[2];                          // the H-apply kernel stages its planes by tensor-map copies (needs HArgs::tmX)
 };
 struct lise_ctx {
     Lattice L;
@@ -333,7 +334,7 @@ static KernSet make_v5_set()
     constexpr int RYZ = TWO_YZ ? v5_maxr(WYZ, 2) : v5_maxr(WYZ, 1), RXZ = TWO_XZ ? v5_maxr(WXZ, 2) : v5_maxr(WXZ, 1);
     constexpr bool WST = !TWO_XZ && BXZ == 2 && v5_smem_happly_xz<NX, NZ>(CXZ, BXZ, WXZ, true) <= SMEM_LIMIT;
     k.h_yz = k5_happly_yz<NY, NZ, CYZ, BYZ, WYZ, VST, RYZ>; k.h_xz = k5_happly_xz<NX, NZ, CXZ, BXZ, WXZ, RXZ, WST>;
-    k.cps_h[0] = TWO_YZ ? 2 : 1; k.cps_h[1] = TWO_XZ ? 2 : 1;
+    k.cps_h[0] = TWO_YZ ? 2 : 1; k.cps_h[1] = TWO_XZ ? 2 : 1; k.tma_h[0] = k.tma_h[1] = 0;
     k.u[0] = nullptr; k.u[1] = k5_update<1>; k.u[2] = k5_update<2>; k.u[3] = k5_update<3>;
     constexpr int SBY = v5_dens_sb<NY, NZ>(), SBX = v5_dens_sb<NX, NZ>();
     k.d_yz = k5_dens_yz<NY, NZ, WDY, SBY>; k.d_x = k5_dens_x<NX, NZ, WDX, SBX>;
@@ -366,13 +367,13 @@ static KernSet make_v6_set()
     static_assert(GY::SMEM <= SMEM_LIMIT, "yz plane too large");
     constexpr bool WHOLE = (CYZ == 4);                         // the yz kernel sees whole states: it adds the pairing block
     k.h_yz = k6_happly_yz<NY, NZ, CYZ, v6_regs(GY::NW, 1), WHOLE>;
-    k.cps_h[0] = 1; k.thr_h[0] = 32 * GY::NW; k.smem_h[0] = GY::SMEM;
+    k.cps_h[0] = 1; k.thr_h[0] = 32 * GY::NW; k.smem_h[0] = GY::SMEM; k.tma_h[0] = 1;
     if (!WHOLE) {
         typedef XZGeom<NX, NZ> GX;
         static_assert(GX::SMEM <= SMEM_LIMIT, "xz plane too large");
         constexpr int CPS_X = (2 * (GX::SMEM + 1024) <= SMEM_SM && 2 * GX::NW <= 16) ? 2 : 1;
         k.h_xz = k6_happly_xz<NX, NZ, v6_regs(GX::NW, CPS_X)>;
-        k.cps_h[1] = CPS_X; k.thr_h[1] = 32 * GX::NW; k.smem_h[1] = GX::SMEM; k.ups_xz = 1;
+        k.cps_h[1] = CPS_X; k.thr_h[1] = 32 * GX::NW; k.smem_h[1] = GX::SMEM; k.ups_xz = 1; k.tma_h[1] = 1;
     }
     k.name = "fft";
     return k;
@@ -401,14 +402,42 @@ static bool pick_kernels(int nx, int ny, int nz, int R, KernSet* out)
     else *out = make_set<DenseLines<2>, DenseLines<2>>("dense");
     out->thr_h[0] = out->thr_h[1] = out->thr_u = out->thr_d = out->thr_dyz = 0;
     out->smem_h[0] = out->smem_h[1] = out->smem_u = out->smem_d = out->smem_dyz = 0;
-    out->ups_xz = 1; out->v5 = 0; out->d_yz = nullptr; out->cps_h[0] = out->cps_h[1] = 1;
+    out->ups_xz = 1; out->v5 = 0; out->d_yz = nullptr; out->cps_h[0] = out->cps_h[1] = 1; out->tma_h[0] = out->tma_h[1] = 0;
     return false;
+}
+
+// tensor map of a wavefunction block X = [ncomp][nx][ny][nz] complex128 for the plane-tile loads of the FFT kernels:
+// elements are doubles, innermost box = 16 doubles = one 128-byte swizzle row; KIND 0: [ny rows][128 B] tiles of a
+// yz-plane, KIND 1: [nx rows][128 B] tiles of an xz-plane (rows at stride ny nz)
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+static int make_plane_tmap(lise_ctx* c, int kind, const cplx* X, int ncomp, CUtensorMap* out)
+{
+    static EncodeTiledFn encode = nullptr;
+    if (!encode) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        CK(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+        if (!fn || qres != cudaDriverEntryPointSuccess) { snprintf(c->err, sizeof(c->err), "cuTensorMapEncodeTiled not available"); return LISE_ECUDA; }
+        encode = (EncodeTiledFn)fn;
+    }
+    const Lattice& L = c->L;
+    const cuuint64_t dims[4] = {(cuuint64_t)2 * L.nz, (cuuint64_t)L.ny, (cuuint64_t)L.nx, (cuuint64_t)(ncomp > 0 ? ncomp : 1)};
+    const cuuint64_t strides[3] = {(cuuint64_t)16 * L.nz, (cuuint64_t)16 * L.nz * L.ny, (cuuint64_t)16 * L.nxyz};
+    const cuuint32_t box[4] = {16u, kind == 0 ? (cuuint32_t)L.ny : 1u, kind == 0 ? 1u : (cuuint32_t)L.nx, 1u};
+    const cuuint32_t estr[4] = {1u, 1u, 1u, 1u};
+    const CUresult r = encode(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, (void*)X, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                              CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) { snprintf(c->err, sizeof(c->err), "cuTensorMapEncodeTiled failed (%d)", (int)r); return LISE_ECUDA; }
+    return LISE_OK;
 }
 
 template <int KIND>
 static int launch_happly(lise_ctx* c, const HArgs& a)
 {
     HArgs b = a;
+    if (c->ks.tma_h[KIND]) TRY(make_plane_tmap(c, KIND, a.X, 4 * a.ns, &b.tmX));
     b.G = c->G * c->ks.cps_h[KIND];
     dim3 grid(KIND == 0 ? c->L.nx : c->L.ny, b.G);
     prof_begin(c, KIND == 0 ? PC_HAPPLY_YZ : PC_HAPPLY_XZ);

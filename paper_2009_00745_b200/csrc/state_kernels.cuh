@@ -127,6 +127,7 @@ __device__ __forceinline__ void stage_table(double2* s, const double2* __restric
 //                                       (H psi)_v = -conj(h conj v) + conj(Delta) (-u_dn, u_up).
 // ------------------------------------------------------------------------------------------------
 struct HArgs {
+    alignas(64) CUtensorMap tmX;   // tensor map of X as [4 ns][nx][ny][2 nz doubles], 128-byte swizzled plane tiles (TMA kernels only)
     Lattice L;
     const cplx* X;
     cplx* W;
