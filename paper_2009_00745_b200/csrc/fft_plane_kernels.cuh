@@ -1,8 +1,8 @@
 // fft_plane_kernels.cuh -- H-apply kernels with the FFT-cost line operator.
 //
 //   k6_happly_yz : W  = [V_loc + T_y + T_z] X (+ pairing block, PAIRING) (yz-plane owner CTAs)
-//   k6_happly_xz : W += T_x X + pairing block, eta partial sums           (xz-plane owner CTAs; lattices whose yz-plane
-//                  units are 2-spinors, where the yz kernel cannot add the pairing block: 32^3)
+//   k6_happly_xz : W += T_x X (+ pairing block), eta partial sums         (xz-plane owner CTAs; the pairing block is added
+//                  here on lattices whose yz-plane units are 2-spinors, where the yz kernel cannot add it: 32^3)
 //
 // Decomposition: h = V_loc + sum_i T_i,
 //   T_i phi = -(1/2) [ M D2_i phi + D2_i (M phi) ] - i [ B_i D_i phi + D_i (B_i phi) ],  B_i = A_i + (sigma x W)_i / 2.
@@ -272,7 +272,7 @@ struct YZGeom {
     static constexpr int NPAIR = NCOMP / 2, UPS = 4 / NCOMP;
     static constexpr int NTY = (NZ + 7) / 8, NTZ = (NY + 7) / 8;
     static constexpr int NWY = NPAIR * NTY, NWZ = NPAIR * NTZ, NW = NWY + NWZ;
-    static constexpr size_t SMEM = 16 * (size_t)PL::SIZE * (2 * NCOMP + NCOMP + 7) + 1024;   // + alignment slack
+    static constexpr size_t SMEM = 16 * (size_t)PL::SIZE * (2 * NCOMP + NCOMP + (NCOMP == 4 ? 7 : 6)) + 1024;   // V3 = Delta only with whole states; + alignment slack
     static constexpr int TCOLS = tmem_cols(NW, NY > NZ ? NY : NZ);
 };
 
@@ -398,64 +398,74 @@ __global__ void __maxnreg__(MAXR) k6_happly_yz(const __grid_constant__ HArgs a)
 }
 
 // ------------------------------------------------------------------------------------------------
-// H-apply, xz-planes:  W += T_x X + pairing block (Eq. 11, mu = 0:  (H psi)_u = h u + Delta (v_dn, -v_up),
+// H-apply, xz-planes:  W += T_x X (+ pairing block with PAIRING: PAPER.md Eq. 11, mu = 0:  (H psi)_u = h u + Delta (v_dn, -v_up),
 // (H psi)_v = -conj(h conj v) + conj(Delta) (-u_dn, u_up));  eta_part[st * ny + iy] = dV Re <X|W> over the plane.
 // grid (ny, G).  A unit = one state; every warp runs one strip of 8 x lines of one 2-spinor per unit; W is read from
 // and written to global memory (row-contiguous 16-byte pairs) in the final loop, all loads in flight at once.
-// mbarriers F[buf] / E[buf] as in k6_happly_yz.   shared: phi[2][4][SIZE] | P1x P2x D [SIZE] | red[2][NW]
+// mbarriers F[buf] / E[buf] per half as in k6_happly_yz.   shared: phi[NH][2][4][SIZE] | P1x P2x D [SIZE] | red[NH][2][NWH]
 // ------------------------------------------------------------------------------------------------
+// NH = units (states) a CTA works on at the same time: each "half" of NW / NH warps runs its own unit pipeline
+// (own buffers and mbarriers) and shares the staged potentials; 2 where the planes are small enough (edges <= 24).
 template <int NX, int NZ>
 struct XZGeom {
     typedef PlaneL<NX, NZ> PL;
-    static constexpr int NTX = (NZ + 7) / 8, NW = 2 * NTX;
-    static constexpr size_t SMEM = 16 * (size_t)PL::SIZE * (2 * 4 + 3) + 1024;
+    static constexpr int NTX = (NZ + 7) / 8, NWH = 2 * NTX;
+    static constexpr int NH = (NWH <= 6 && 16 * (size_t)PL::SIZE * (2 * 2 * 4 + 3) + 1024 <= 180 * 1024) ? 2 : 1;
+    static constexpr int NW = NH * NWH;
+    static constexpr size_t SMEM = 16 * (size_t)PL::SIZE * (NH * 2 * 4 + 3) + 1024;
     static constexpr int TCOLS = tmem_cols(NW, NX);
 };
 
-template <int NX, int NZ, int MAXR>
+template <int NX, int NZ, int MAXR, bool PAIRING>
 __global__ void __maxnreg__(MAXR) k6_happly_xz(const __grid_constant__ HArgs a)
 {
     typedef XZGeom<NX, NZ> G;
     typedef typename G::PL PL;
     constexpr int NPTS = NX * NZ, SZ = PL::SIZE, TS = PL::TS, SZB = SZ * 16;
-    constexpr int NW = G::NW, NTHR = NW * 32;
+    constexpr int NW = G::NW, NTHR = NW * 32, NH = G::NH, NWH = G::NWH, NTHRH = NWH * 32;
     extern __shared__ unsigned char smem_raw[];
     const unsigned s_raw = smem_u32(smem_raw), s_phi = (s_raw + 1023u) & ~1023u;
     cplx* phi = (cplx*)(smem_raw + (s_phi - s_raw));
-    double2* P1x = phi + 2 * 4 * SZ;
+    double2* P1x = phi + NH * 2 * 4 * SZ;
     double2 *P2x = P1x + SZ, *Dl = P2x + SZ;
-    const unsigned s_px = s_phi + 2 * 4 * SZB;
+    const unsigned s_px = s_phi + NH * 2 * 4 * SZB;
     __shared__ double s_red[2 * NW];
-    __shared__ unsigned long long s_bar[4];
+    __shared__ unsigned long long s_bar[4 * NH];
     __shared__ unsigned s_tmem;
-    unsigned long long *barF = s_bar, *barE = s_bar + 2;
     const int nxyz = a.L.nxyz, gs = a.L.ny * NZ, gb = blockIdx.x * NZ;
     const double* pot = a.pot;
     const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
+    const int half = warp / NWH, wh = warp - half * NWH;
+    const bool leader = threadIdx.x == half * NTHRH;                  // first thread of the half: stages units, writes eta
+    unsigned long long *barF = s_bar + 4 * half, *barE = barF + 2;
+    double* red = s_red + 2 * NWH * half;
     if (threadIdx.x == 0) {
-        mbar_init(barF, 1); mbar_init(barF + 1, 1);
-        mbar_init(barE, NTHR); mbar_init(barE + 1, NTHR);
+        for (int h = 0; h < NH; ++h) {
+            mbar_init(s_bar + 4 * h, 1); mbar_init(s_bar + 4 * h + 1, 1);
+            mbar_init(s_bar + 4 * h + 2, NTHRH); mbar_init(s_bar + 4 * h + 3, NTHRH);
+        }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     const unsigned tbase = tmem_alloc<G::TCOLS>(&s_tmem, warp);
     const unsigned tr = tbase + ((unsigned)(warp & 3) << 21) + (unsigned)(warp >> 2) * (2 * NX);
-    const int nunits = a.ns;
-    // one thread stages a unit: 4 x NT tensor-map tile copies ([NX rows at stride ny nz][128 bytes], hardware-swizzled)
+    const int nunits = a.ns, ustep = a.G * NH;
+    const unsigned s_half = s_phi + half * 2 * 4 * SZB;
+    // one thread per half stages a unit: 4 x NT tensor-map tile copies ([NX rows at stride ny nz][128 bytes], hardware-swizzled)
     auto issue = [&](int u, int buf) {
-        if (threadIdx.x != 0) return;
+        if (!leader) return;
         mbar_expect_tx(barF + buf, 4 * PL::NT * NX * 128);
 #pragma unroll
         for (int c = 0; c < 4; ++c)
 #pragma unroll
             for (int t = 0; t < PL::NT; ++t)
-                tma_load_tile(s_phi + ((buf * 4 + c) * SZ + t * TS) * 16, &a.tmX, barF + buf, 16 * t, (int)blockIdx.x, 0, u * 4 + c);
+                tma_load_tile(s_half + ((buf * 4 + c) * SZ + t * TS) * 16, &a.tmX, barF + buf, 16 * t, (int)blockIdx.x, 0, u * 4 + c);
     };
-    auto flush_eta = [&](int uprev, int it_prev) {               // thread 0: fixed-order sum of the warps' partials
+    auto flush_eta = [&](int uprev, int it_prev) {               // leader: fixed-order sum of the warps' partials
         double s = 0.0;
-        for (int w = 0; w < NW; ++w) s += s_red[(it_prev & 1) * NW + w];
+        for (int w = 0; w < NWH; ++w) s += red[(it_prev & 1) * NWH + w];
         a.eta_part[(size_t)uprev * a.L.ny + blockIdx.x] = s * a.L.dV;
     };
-    int u = blockIdx.y, uprev = -1;
+    int u = blockIdx.y * NH + half, uprev = -1;
     if (u < nunits) issue(u, 0);
     {
         const double i1 = 1.0 / a.L.dx, i2 = i1 * i1;
@@ -468,7 +478,7 @@ __global__ void __maxnreg__(MAXR) k6_happly_xz(const __grid_constant__ HArgs a)
     }
     __syncthreads();
 
-    const int pr = warp / G::NTX, strip = warp - pr * G::NTX;    // pr = pair: 0 the u pair, 1 the v pair (phi = conj v)
+    const int pr = wh / G::NTX, strip = wh - pr * G::NTX;        // pr = pair: 0 the u pair, 1 the v pair (phi = conj v)
     LaneRole ln; ln.init();
     const int line_raw = 8 * strip + ln.j;
     const bool valid = line_raw < NZ;
@@ -480,17 +490,24 @@ __global__ void __maxnreg__(MAXR) k6_happly_xz(const __grid_constant__ HArgs a)
     const int oc = 2 * (1 - pr) + (1 - ln.s);
     const unsigned fa = pr ? (ln.sm ^ 0x80000000u) : ln.sm, fb = pr ? ln.pm : (ln.pm ^ 0x80000000u);
     int it = 0;
-    for (; u < nunits; u += a.G, ++it) {
+    for (; u < nunits; u += ustep, ++it) {
         const int buf = it & 1;
         mbar_wait(barF + buf, (it >> 1) & 1);
-        const unsigned s_unit = s_phi + buf * 4 * SZB;
+        const unsigned s_unit = s_half + buf * 4 * SZB;
         const unsigned b_w = LA::base(s_unit + 2 * pr * SZB, line);
         auto mid = [&]() {
             if (it >= 1) {
-                mbar_wait(barE + (buf ^ 1), ((it - 1) >> 1) & 1);    // everyone is done with unit u - G
-                if (threadIdx.x == 0) flush_eta(uprev, it - 1);
+                mbar_wait(barE + (buf ^ 1), ((it - 1) >> 1) & 1);    // this half is done with unit u - ustep
+                if (leader) flush_eta(uprev, it - 1);
             }
-            if (u + a.G < nunits) issue(u + a.G, buf ^ 1);
+            if (u + ustep < nunits) {
+                issue(u + ustep, buf ^ 1);
+                // the next unit's W values of this thread's points: into L2 now, so that the loads below do not wait for
+                // HBM while the ABM update streams beside this CTA
+                const double* wn = (const double*)(a.W + ((size_t)(u + ustep) * 4 + 2 * pr + ln.s) * nxyz + gb + line) + ln.p;
+#pragma unroll
+                for (int i = 0; i < NX; ++i) asm volatile("prefetch.global.L2 [%0];" ::"l"(wn + (size_t)i * gs * 2));
+            }
         };
         double cc[NX];
         line_task6<NX, 0, true, TS, SZB, false, 0>(b_w, b_pot, cj, ln, tr, cc, mid);
@@ -512,18 +529,20 @@ __global__ void __maxnreg__(MAXR) k6_happly_xz(const __grid_constant__ HArgs a)
         static_for<NX>([&](auto ic) {
             constexpr int i = decltype(ic)::value, e = line_ord(i, NX);
             constexpr int K = LA::k16(e), I = LA::imm(e);
-            const double2 dl = lds_v2<K, I + 2 * SZB>(b_pot);
-            const double o2 = lds_f64<K, I>(b_o), o3 = lds_f64<K, I>(b_o ^ 8u);
             double w = win[i] + cc[i];
-            w += flip(fma(flip(dl.y, fb), o3, dl.x * o2), fa);
+            if (PAIRING) {
+                const double2 dl = lds_v2<K, I + 2 * SZB>(b_pot);
+                const double o2 = lds_f64<K, I>(b_o), o3 = lds_f64<K, I>(b_o ^ 8u);
+                w += flip(fma(flip(dl.y, fb), o3, dl.x * o2), fa);
+            }
             if (valid) { __stcg(Wg + (size_t)e * gs * 2, w); eta = fma(lds_f64<K, I>(b_x), w, eta); }
         });
         for (int o = 16; o > 0; o >>= 1) eta += __shfl_xor_sync(0xffffffffu, eta, o);
-        if ((threadIdx.x & 31) == 0) s_red[(it & 1) * NW + warp] = eta;
+        if ((threadIdx.x & 31) == 0) red[(it & 1) * NWH + wh] = eta;
         mbar_arrive(barE + buf);
         uprev = u;
     }
     __syncthreads();
-    if (threadIdx.x == 0 && uprev >= 0) flush_eta(uprev, it - 1);
+    if (leader && uprev >= 0) flush_eta(uprev, it - 1);
     tmem_free<G::TCOLS>(tbase, warp);
 }

@@ -346,35 +346,31 @@ static KernSet make_v5_set()
     return k;
 }
 // ---- FFT-cost line operator (fft_plane_kernels.cuh): one real line per thread, generated real-input FFT codelets.
-// Lattices with every edge in {8, 12, 16, 20, 24, 32}.  Where a whole state fits the yz-plane CTA's shared memory
-// (edges <= 24) the FFT kernel runs the y and z lines and the pairing block, and the x lines stay with the DMMA kernel
-// k5_happly_xz: capped at 128 registers, it leaves room for the co-resident ABM update CTA (measured on config 1:
-// 59.5 ms per step against 63.4 ms with both H-apply kernels on the FFT path and 60.6 ms with both on DMMA).  At 32^3
-// (2-spinor units) both H-apply kernels are the FFT ones (162.9 against 170.0 ms per step).  The ABM update and the
-// density kernels are those of plane5_kernels.cuh.
-static constexpr size_t SMEM_SM = 228 * 1024;                 // shared memory of one SM; 1 KB per resident CTA is reserved
-static constexpr int v6_regs(int warps, int ctas)
+// Lattices with every edge in {8, 12, 16, 20, 24, 32}.  Both H-apply kernels are the FFT ones; where a whole state fits
+// the yz-plane CTA's shared memory (edges <= 24) the yz kernel adds the pairing block, else (32^3, 2-spinor units) the
+// xz kernel does.  The ABM update is k7_update, co-resident with them; the density kernels and the starter's update
+// are those of plane5_kernels.cuh.
+static constexpr int v6_regs(int warps)
 {
-    const int r = (65536 / (warps * 32 * ctas)) & ~7;
+    const int r = (65536 / (warps * 32)) & ~7;
     return r > 255 ? 255 : r;
 }
 template <int NX, int NY, int NZ>
 static KernSet make_v6_set()
 {
-    KernSet k = make_v5_set<NX, NY, NZ>();                     // update, density and (whole-state units) xz kernels
+    KernSet k = make_v5_set<NX, NY, NZ>();                     // update and density kernels
     constexpr int CYZ = (YZGeom<NY, NZ, 4>::SMEM <= SMEM_LIMIT) ? 4 : 2;
     typedef YZGeom<NY, NZ, CYZ> GY;
+    typedef XZGeom<NX, NZ> GX;
     static_assert(GY::SMEM <= SMEM_LIMIT, "yz plane too large");
+    static_assert(GX::SMEM <= SMEM_LIMIT, "xz plane too large");
     constexpr bool WHOLE = (CYZ == 4);                         // the yz kernel sees whole states: it adds the pairing block
-    k.h_yz = k6_happly_yz<NY, NZ, CYZ, v6_regs(GY::NW, 1), WHOLE>;
+    // the yz kernel takes every register of the SM (its shared-memory pipe is the busiest unit: nothing gains from a
+    // neighbour); the xz kernel leaves one warp of LISE_UPD_REGS registers per sub-partition to the update CTA
+    k.h_yz = k6_happly_yz<NY, NZ, CYZ, v6_regs(GY::NW), WHOLE>;
     k.cps_h[0] = 1; k.thr_h[0] = 32 * GY::NW; k.smem_h[0] = GY::SMEM; k.tma_h[0] = 1;
-    if (!WHOLE) {
-        typedef XZGeom<NX, NZ> GX;
-        static_assert(GX::SMEM <= SMEM_LIMIT, "xz plane too large");
-        constexpr int CPS_X = (2 * (GX::SMEM + 1024) <= SMEM_SM && 2 * GX::NW <= 16) ? 2 : 1;
-        k.h_xz = k6_happly_xz<NX, NZ, v6_regs(GX::NW, CPS_X)>;
-        k.cps_h[1] = CPS_X; k.thr_h[1] = 32 * GX::NW; k.smem_h[1] = GX::SMEM; k.ups_xz = 1; k.tma_h[1] = 1;
-    }
+    k.h_xz = k6_happly_xz<NX, NZ, coresident_regs(GX::NW), !WHOLE>;
+    k.cps_h[1] = 1; k.thr_h[1] = 32 * GX::NW; k.smem_h[1] = GX::SMEM; k.ups_xz = 1; k.tma_h[1] = 1;
     k.name = "fft";
     return k;
 }

@@ -474,12 +474,13 @@ __global__ void __maxnreg__(MAXR) k5_happly_xz(HArgs a)
 //   MODE 3 (starter, Taylor term `order`): as k_update_yz<3> in state_kernels.cuh
 // History slots are read and written with streaming cache hints so that W, X and the new state stay in L2.
 // ------------------------------------------------------------------------------------------------
-// 128 threads and <= 128 registers: one CTA fits beside a 12-warp, 128-register H-apply CTA on the same SM, so the
-// update of chunk i streams from HBM while the tensor-core kernels of chunk i + 1 run.
+// 128 threads (one warp per SM sub-partition) and <= LISE_UPD_REGS registers: one CTA fits beside a plane-owner CTA
+// capped at coresident_regs() registers on the same SM, so the update of chunk i streams from HBM while the x-line
+// H-apply and the density kernels of the neighbouring chunks run.
 #define LISE_UPD_THREADS 128
-template <int MODE> struct UpdEpt { static constexpr int V = (MODE == 1) ? 3 : (MODE == 2) ? 6 : 2; };   // elements per thread
+template <int MODE> struct UpdEpt { static constexpr int V = (MODE == 1) ? 2 : (MODE == 2) ? 4 : 2; };   // elements per thread
 template <int MODE>
-__global__ void __launch_bounds__(LISE_UPD_THREADS) k5_update(UArgs a)
+__global__ void __maxnreg__(LISE_UPD_REGS) k5_update(UArgs a)
 {
     __shared__ double s_eta;
     const int st = blockIdx.y;
@@ -657,7 +658,7 @@ __device__ __forceinline__ void dens_task_flush5(double* __restrict__ part, int 
 // at the end, map by map (deterministic).   shared: tables | v[2][SB][2][PP]
 // ------------------------------------------------------------------------------------------------
 template <int NY, int NZ, int NWARP, int SB>
-__global__ void __launch_bounds__(NWARP * 32, 1) k5_dens_yz(DArgs a)
+__global__ void __maxnreg__(coresident_regs(NWARP)) k5_dens_yz(DArgs a)
 {
     extern __shared__ double2 smem[];
     constexpr int LD = ldpad(NZ), PP = NY * LD, NPTS = NY * NZ, NTHR = NWARP * 32;
@@ -781,7 +782,7 @@ __global__ void __launch_bounds__(NWARP * 32, 1) k5_dens_yz(DArgs a)
 
 // x-axis density pass of the states in Z.   grid (ny, G), NWARP warps.  shared: table | v[2][2][PP]
 template <int NX, int NZ, int NWARP, int SB>
-__global__ void __launch_bounds__(NWARP * 32, 1) k5_dens_x(DArgs a)
+__global__ void __maxnreg__(coresident_regs(NWARP)) k5_dens_x(DArgs a)
 {
     extern __shared__ double2 smem[];
     constexpr int LD = ldpad(NZ), PP = NX * LD, NPTS = NX * NZ;

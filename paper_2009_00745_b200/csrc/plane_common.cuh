@@ -7,6 +7,15 @@
 #include "common.cuh"
 #include "state_kernels.cuh"
 
+// Register budget of a plane-owner CTA that is to share its SM with the ABM update CTA (k5_update: 4 warps, one per
+// SM sub-partition, <= LISE_UPD_REGS registers).  The register file is per sub-partition (16384 registers each), so
+// the budget is per sub-partition too: (warps / 4) x 32 x R + 32 x LISE_UPD_REGS <= 16384.
+#define LISE_UPD_REGS 80
+__host__ __device__ constexpr int coresident_regs(int warps)
+{
+    const int r = ((16384 - 32 * LISE_UPD_REGS) / (((warps + 3) / 4) * 32)) & ~7;
+    return r > 255 ? 255 : r;
+}
 __host__ __device__ constexpr int ldpad(int n) { return n + ((4 - n % 8) + 8) % 8; }
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc)
