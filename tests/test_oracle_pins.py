@@ -491,6 +491,48 @@ def test_free_two_mode_state_exact_phase():
     assert np.abs(got2[0, 0] - w2).max() / np.abs(w2).max() < 1e-8
 
 
+def test_stepper_is_the_scalar_linear_recurrence_of_eq78_to_roundoff():
+    """SURVEY 8(c) "ABM linear recurrence": interaction and phase removal off, one plane-wave state: H psi = E psi
+    with a constant E, so the whole stepper (3 starter steps = multiplication by the 4th-order series T4(z), Eq. 77,
+    then Eqs. 78a-d with its history rotation and e_3 = 0, reading B18) is a linear recurrence in one complex
+    amplitude.  The recurrence is run here in scalar Python arithmetic and must agree to round-off, not to the
+    truncation error: a swapped history slot, a stale e_n or a wrong hand-off from the starter fails at 1e-9."""
+    shape, a, dt = (6, 4, 8), 1.25, 0.05
+    par = _free_params()
+    par.remove_phase = 0
+    c = ref.RefContext(*shape, a, dt, 1, 0, params=par)
+    x = np.meshgrid(*[np.arange(n) * a for n in shape], indexing="ij")
+    Ls = [n * a for n in shape]
+    k = np.array([2 * np.pi * 2 / Ls[0], 2 * np.pi * 1 / Ls[1], 2 * np.pi * -3 / Ls[2]])
+    psi = np.zeros((1, 4) + shape, complex)
+    psi[0, 1] = np.exp(1j * sum(qi * xi for qi, xi in zip(k, x))) / math.sqrt(np.prod(Ls))
+    c.set_wavefunctions(0, psi)
+    lam = -1j * par.hbar2_2m * (k @ k) / par.hbarc           # y' = lam y  (Eq. 80 with eta = 0, u component)
+    z = lam * dt
+    T4 = 1 + z + z ** 2 / 2 + z ** 3 / 6 + z ** 4 / 24
+    ys = [1.0 + 0j]
+    for _ in range(3):
+        ys.append(T4 * ys[-1])
+    fs = [lam * y for y in ys]                               # f_0 .. f_3
+    e = 0.0
+    nabm = 9
+    for n in range(3, 3 + nabm):
+        pn = (ys[n] + ys[n - 1]) / 2 + dt / 48 * (119 * fs[n] - 99 * fs[n - 1] + 69 * fs[n - 2] - 17 * fs[n - 3])
+        mn = pn - 161 / 170 * e
+        cn = (ys[n] + ys[n - 1]) / 2 + dt / 48 * (17 * lam * mn + 51 * fs[n] + 3 * fs[n - 1] + fs[n - 2])
+        e = pn - cn
+        ys.append(cn + 9 / 170 * e)
+        fs.append(lam * ys[-1])
+    c.step(3 + nabm)
+    got = c.get_wavefunctions(0)
+    want = psi[0, 1] * ys[-1]
+    assert np.abs(got[0, 1] - want).max() / np.abs(want).max() < 2e-13
+    assert np.abs(got[0, [0, 2, 3]]).max() < 1e-15
+    # and the recurrence itself tracks e^{lam t} within the method's error (so the pin is not vacuous)
+    t = (3 + nabm) * dt
+    assert abs(ys[-1] - np.exp(lam * t)) < 5 * (3 * abs(z) ** 5 / 120 + nabm * 0.0098 * abs(z) ** 6)
+
+
 @pytest.fixture(scope="module")
 def evolved_small():
     """config-0-like small problem: both species, Coulomb, pairing, 10 steps."""
