@@ -1,7 +1,7 @@
 // lise.cu -- C-ABI entry points (include/lise.h) and host-side orchestration of the TDSLDA step.
 //
 // Resident state arrays per species ("slots", roles rotate by pointer swap):
-//   A y_n | B y_{n-1} -> Q -> y_{n+1} | C f_{n-3} -> f_n | D f_{n-1} | E f_{n-2} | F e_n -> m -> e_{n+1} | G p
+//   A y_n | B y_{n-1} -> Q -> y_{n+1} | C f_{n-3} -> f_n | D f_{n-1} | E f_{n-2} | F e_n -> e_{n+1} | G m
 // One ABM step (Eq. 78) = two evaluations; each evaluation = grid-only potentials, then per
 // chunk of states: k_happly<0> (yz-planes) -> k_happly<1> (xz-planes, eta) -> k_update_yz (ABM + y/z
 // densities of the new state) -> k_dens_x (x densities of the new state).
@@ -662,7 +662,7 @@ static int abm_step(lise_ctx* c)
         auto flush_dens = [&](int last_chunk) -> int {
             if (pend_q < 0) return LISE_OK;
             if (pipe) CK(cudaStreamWaitEvent(c->stream, c->ev_u[last_chunk & 1], 0));
-            TRY(dens_chunk(c, pend_q, (phase == 1 ? S(c, pend_q, RF) : S(c, pend_q, RB)) + pend_off, pend_ns));
+            TRY(dens_chunk(c, pend_q, (phase == 1 ? S(c, pend_q, RG) : S(c, pend_q, RB)) + pend_off, pend_ns));
             pend_q = -1; pend_ns = 0; pend_chunks = 0;
             return LISE_OK;
         };
@@ -671,7 +671,7 @@ static int abm_step(lise_ctx* c)
                 const int ns = (c->nwf[q] - s0 < c->chunk) ? c->nwf[q] - s0 : c->chunk;
                 const size_t off = s0 * slen;
                 const int wb = pipe ? (i & 1) : 0;
-                const cplx* X = (phase == 1 ? S(c, q, RA) : S(c, q, RF)) + off;
+                const cplx* X = (phase == 1 ? S(c, q, RA) : S(c, q, RG)) + off;
                 if (pipe && i >= 2) CK(cudaStreamWaitEvent(c->stream, c->ev_u[wb], 0));   // W[wb], eta[wb] are free again
                 TRY(apply_h_chunk(c, q, X, Wbuf(c, wb), etabuf(c, wb), ns));
                 UArgs u = make_uargs(c, q, off, ns, wb);
@@ -685,7 +685,7 @@ static int abm_step(lise_ctx* c)
                     if (pend_q < 0) { pend_q = q; pend_off = off; }
                     pend_ns += ns; pend_chunks += 1;
                 } else {
-                    TRY(launch_dens_x(c, make_dargs(c, q, (phase == 1 ? S(c, q, RF) : S(c, q, RB)) + off, ns)));
+                    TRY(launch_dens_x(c, make_dargs(c, q, (phase == 1 ? S(c, q, RG) : S(c, q, RB)) + off, ns)));
                 }
             }
         TRY(flush_dens(i - 1));

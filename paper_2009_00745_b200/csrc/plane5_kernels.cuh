@@ -469,8 +469,10 @@ __global__ void __maxnreg__(MAXR) k5_happly_xz(HArgs a)
 
 // ------------------------------------------------------------------------------------------------
 // ABM update, pure streaming (Eq. 78, Eqs. 80-81).  grid (blocks over the 4 nxyz elements of a state, ns).
-//   MODE 1 (after evaluation 1): f_n = -i (W - eta y_n) / hbar c;  p, Q, m = p - (161/170) e;  C <- f_n, F <- m, G <- p, B <- Q
-//   MODE 2 (after evaluation 2): f_m; c = Q + (dt/48) 17 f_m; e' = p - c; y_{n+1} = c + (9/170) e';  B <- y_{n+1}, F <- e'
+//   MODE 1 (after evaluation 1): f_n = -i (W - eta y_n) / hbar c;  p, Q, m = p - (161/170) e;  C <- f_n, G <- m, B <- Q
+//   MODE 2 (after evaluation 2): f_m; c = Q + (dt/48) 17 f_m; p = m + (161/170) e; e' = p - c; y_{n+1} = c + (9/170) e';
+//           B <- y_{n+1}, F <- e'.   The predictor p is not stored: Eq. 78b is solved for it (one rounding), which saves
+//           one of the 17 array passes of a step.
 //   MODE 3 (starter, Taylor term `order`): as k_update_yz<3> in state_kernels.cuh
 // History slots are read and written with streaming cache hints so that W, X and the new state stay in L2.
 // ------------------------------------------------------------------------------------------------
@@ -524,17 +526,17 @@ __global__ void __maxnreg__(LISE_UPD_REGS) k5_update(UArgs a)
             qq.x = half.x + c48 * (51.0 * fn.x + 3.0 * f1[k].x + f2[k].x);
             qq.y = half.y + c48 * (51.0 * fn.y + 3.0 * f1[k].y + f2[k].y);
             const cplx m = cmk(pp.x - (161.0 / 170.0) * e[k].x, pp.y - (161.0 / 170.0) * e[k].y);
-            __stcs(a.sC + o, fn); __stcs(a.sG + o, pp); __stcs(a.sB + o, qq);
-            a.sF[o] = m;                                    // the new state: read again by the density kernels
+            __stcs(a.sC + o, fn); __stcs(a.sB + o, qq);
+            a.sG[o] = m;                                    // the new state: read again by the density kernels
         }
     } else if (MODE == 2) {
-        cplx w[LISE_UPD_EPT], m[LISE_UPD_EPT], qq[LISE_UPD_EPT], pp[LISE_UPD_EPT];
+        cplx w[LISE_UPD_EPT], m[LISE_UPD_EPT], qq[LISE_UPD_EPT], en[LISE_UPD_EPT];
 #pragma unroll
         for (int k = 0; k < LISE_UPD_EPT; ++k) {
             const size_t el = e0 + (size_t)k * LISE_UPD_THREADS;
             if (el >= slen) continue;
             const size_t o = so + el;
-            w[k] = __ldcs(a.W + o); m[k] = __ldcs(a.sF + o); qq[k] = __ldcs(a.sB + o); pp[k] = __ldcs(a.sG + o);
+            w[k] = __ldcs(a.W + o); m[k] = __ldcs(a.sG + o); qq[k] = __ldcs(a.sB + o); en[k] = __ldcs(a.sF + o);
         }
 #pragma unroll
         for (int k = 0; k < LISE_UPD_EPT; ++k) {
@@ -543,7 +545,8 @@ __global__ void __maxnreg__(LISE_UPD_REGS) k5_update(UArgs a)
             const size_t o = so + el;
             const cplx fm = cmk((w[k].y - eta * m[k].y) * ih, -(w[k].x - eta * m[k].x) * ih);
             const cplx cc = cmk(qq[k].x + c48 * 17.0 * fm.x, qq[k].y + c48 * 17.0 * fm.y);
-            const cplx ee = cmk(pp[k].x - cc.x, pp[k].y - cc.y);
+            const cplx pp = cmk(m[k].x + (161.0 / 170.0) * en[k].x, m[k].y + (161.0 / 170.0) * en[k].y);   // Eq. 78b solved for p
+            const cplx ee = cmk(pp.x - cc.x, pp.y - cc.y);
             const cplx yn = cmk(cc.x + (9.0 / 170.0) * ee.x, cc.y + (9.0 / 170.0) * ee.y);
             __stcs(a.sF + o, ee);
             a.sB[o] = yn;

@@ -287,8 +287,9 @@ __device__ __forceinline__ void dens_axis_rmw(double* part, int nxyz, int gi, in
 //            p = (y_n + y_{n-1})/2 + dt/48 (119 f_n - 99 f_{n-1} + 69 f_{n-2} - 17 f_{n-3})   (Eq. 78a)
 //            m = p - 161/170 e_n                                                              (Eq. 78b)
 //            Q = (y_n + y_{n-1})/2 + dt/48 (51 f_n + 3 f_{n-1} + f_{n-2})   [part of Eq. 78c]
-//            writes f_n -> sC (was f_{n-3}), m -> sF (was e_n), p -> sG, Q -> sB (was y_{n-1}); new state = m
+//            writes f_n -> sC (was f_{n-3}), m -> sG, Q -> sB (was y_{n-1}); new state = m; e_n stays in sF
 //   MODE 2 (after evaluation 2, W = H m):  m' = -i (W - eta m)/hbar c; c = Q + dt/48 17 m'    (Eq. 78c)
+//            p = m + 161/170 e_n (Eq. 78b solved for p: p is not stored)
 //            y_{n+1} = c + 9/170 (p - c) -> sB, e_{n+1} = p - c -> sF                          (Eq. 78d); new state = y_{n+1}
 //   MODE 3 (series expansion, Eqs. 75-77): g = -i (W - eta T)/hbar c with T = sA (order 1) or sG;
 //            order 1: eta fixed := eta_k, f_n = g -> sC, T' = dt g -> sG, acc = sA + T' -> sF
@@ -366,9 +367,10 @@ __global__ void __launch_bounds__(LO::MAXT) k_update_yz(UArgs a)
                     qq.x = half.x + c48 * (51.0 * fn.x + 3.0 * f1.x + f2.x);
                     qq.y = half.y + c48 * (51.0 * fn.y + 3.0 * f1.y + f2.y);
                     nw = cmk(pp.x - (161.0 / 170.0) * e.x, pp.y - (161.0 / 170.0) * e.y);
-                    a.sC[o] = fn; a.sF[o] = nw; a.sG[o] = pp; a.sB[o] = qq;
+                    a.sC[o] = fn; a.sG[o] = nw; a.sB[o] = qq;
                 } else if (MODE == 2) {
-                    const cplx w = a.W[o], m = a.sF[o], qq = a.sB[o], pp = a.sG[o];
+                    const cplx w = a.W[o], m = a.sG[o], qq = a.sB[o], en = a.sF[o];
+                    const cplx pp = cmk(m.x + (161.0 / 170.0) * en.x, m.y + (161.0 / 170.0) * en.y);   // Eq. 78b solved for p
                     const cplx fm = cmk((w.y - eta * m.y) * ih, -(w.x - eta * m.x) * ih);
                     const cplx cc = cmk(qq.x + c48 * 17.0 * fm.x, qq.y + c48 * 17.0 * fm.y);
                     const cplx ee = cmk(pp.x - cc.x, pp.y - cc.y);
