@@ -296,13 +296,9 @@ static constexpr int imax(int a, int b) { return a > b ? a : b; }
 // warps per 2-spinor of an H-apply CTA: one strip task per warp if possible; long lines need more registers per thread
 static constexpr int v5_wpp(int npair, int strips, int nline) { return imin(strips, (nline >= 40 ? 8 : 12) / npair); }
 
-// register cap of an H-apply kernel with `warps` warps and `ctas` CTAs per SM; 4 warps x 128 registers stay free for
-// the co-resident update CTA
-static constexpr int v5_maxr(int warps, int ctas)
-{
-    const int r = ((65536 - 4 * 32 * 128) / (warps * 32 * ctas)) & ~7;
-    return r > 255 ? 255 : r;
-}
+// register cap of a DMMA H-apply kernel with `warps` warps and `ctas` CTAs per SM: what leaves room for the co-resident
+// update CTA (plane_common.cuh: coresident_regs, the budget is per SM sub-partition)
+static constexpr int v5_maxr(int warps, int ctas) { return coresident_regs(warps * ctas); }
 // warps for `tasks` equal tasks per pass: all of them if they fit under `cap`, else the largest count <= cap that
 // divides them evenly
 static constexpr int v5_warps(int tasks, int cap)

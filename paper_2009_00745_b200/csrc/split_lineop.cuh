@@ -104,6 +104,51 @@ struct RDFT<4> {
     }
 };
 
+#define LISE_COS72 0.30901699437494742410
+#define LISE_COS144 (-0.80901699437494742410)
+#define LISE_SIN72 0.95105651629515357212
+#define LISE_SIN144 0.58778525229247312917
+template <>
+struct RDFT<5> {                                   // spectral order b0, b1, e1, b2, e2
+    static __device__ __forceinline__ void fwd(const double (&x)[5], double (&v)[5])
+    {
+        const double p14 = x[1] + x[4], m14 = x[1] - x[4], p23 = x[2] + x[3], m23 = x[2] - x[3];
+        v[0] = x[0] + p14 + p23;
+        v[1] = fma(LISE_COS72, p14, fma(LISE_COS144, p23, x[0]));
+        v[2] = fma(LISE_SIN72, m14, LISE_SIN144 * m23);
+        v[3] = fma(LISE_COS144, p14, fma(LISE_COS72, p23, x[0]));
+        v[4] = fma(LISE_SIN144, m14, -LISE_SIN72 * m23);
+    }
+    static __device__ __forceinline__ void inv(const double (&a)[5], double (&y)[5])
+    {
+        const double A1 = fma(LISE_COS72, a[1], fma(LISE_COS144, a[3], a[0])), B1 = fma(LISE_SIN72, a[2], LISE_SIN144 * a[4]);
+        const double A2 = fma(LISE_COS144, a[1], fma(LISE_COS72, a[3], a[0])), B2 = fma(LISE_SIN144, a[2], -LISE_SIN72 * a[4]);
+        y[0] = a[0] + a[1] + a[3]; y[1] = A1 + B1; y[2] = A2 + B2; y[3] = A2 - B2; y[4] = A1 - B1;
+    }
+};
+#define LISE_SQRT_HALF 0.70710678118654752440
+template <>
+struct RDFT<8> {                                   // spectral order b0, b1, e1, b2, e2, b3, e3, b4
+    static __device__ __forceinline__ void fwd(const double (&x)[8], double (&v)[8])
+    {
+        const double s04 = x[0] + x[4], d04 = x[0] - x[4], s26 = x[2] + x[6], d26 = x[2] - x[6];
+        const double s15 = x[1] + x[5], d15 = x[1] - x[5], s37 = x[3] + x[7], d37 = x[3] - x[7];
+        const double se = s04 + s26, so = s15 + s37;
+        const double u = LISE_SQRT_HALF * (d15 - d37), w = LISE_SQRT_HALF * (d15 + d37);
+        v[0] = se + so; v[1] = d04 + u; v[2] = d26 + w; v[3] = s04 - s26;
+        v[4] = s15 - s37; v[5] = d04 - u; v[6] = w - d26; v[7] = se - so;
+    }
+    static __device__ __forceinline__ void inv(const double (&a)[8], double (&y)[8])
+    {
+        const double p0 = a[0] + a[7], p1 = a[0] - a[7];
+        const double e0 = p0 + a[3], e2 = p0 - a[3], o1 = p1 + a[4], o3 = p1 - a[4];
+        const double s13 = a[1] + a[5], d13 = a[1] - a[5], s26 = a[2] + a[6], d26 = a[2] - a[6];
+        const double t1 = LISE_SQRT_HALF * (d13 + s26), t3 = LISE_SQRT_HALF * (s26 - d13);
+        y[0] = e0 + s13; y[4] = e0 - s13; y[2] = e2 + d26; y[6] = e2 - d26;
+        y[1] = o1 + t1; y[5] = o1 - t1; y[3] = o3 + t3; y[7] = o3 - t3;
+    }
+};
+
 // ---- Toeplitz fragments of one operator (op = 0: D, 1: D2) for this thread (g = lane / 4, t = lane % 4) ----
 // fragment f <-> (2 r - kk) = f - (NKH - 1):  A[g][t] = P_j[(8 r + g) - (4 kk + t)]
 template <int N>
