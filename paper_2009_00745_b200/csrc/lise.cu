@@ -294,8 +294,17 @@ static constexpr int v5_dens_sb() { return (16 * (size_t)(4 * 4 * N1 * ldpad(NZ)
 static constexpr int imin(int a, int b) { return a < b ? a : b; }
 static constexpr int imax(int a, int b) { return a > b ? a : b; }
 // warps per 2-spinor of an H-apply CTA: one strip task per warp if possible; long lines need more registers per thread
-static constexpr int v5_wpp(int npair, int strips, int nline) { return imin(strips, (nline >= 40 ? 8 : 12) / npair); }
+// warps a CTA may have for lines of `nline` points (long lines need more registers per thread)
+static constexpr int v5_wcap(int nline) { return nline >= 48 ? 8 : nline >= 40 ? 10 : 12; }
+static constexpr int v5_wpp(int npair, int strips, int nline) { return imin(strips, v5_wcap(nline) / npair); }
 
+// every register of the SM for a CTA of `warps` warps that runs without a neighbour: the register file is per
+// sub-partition (16384 each), which ceil(warps / 4) warps share
+static constexpr int v6_regs(int warps)
+{
+    const int r = (16384 / (((warps + 3) / 4) * 32)) & ~7;
+    return r > 255 ? 255 : r;
+}
 // register cap of a DMMA H-apply kernel with `warps` warps and `ctas` CTAs per SM: what leaves room for the co-resident
 // update CTA (plane_common.cuh: coresident_regs, the budget is per SM sub-partition)
 static constexpr int v5_maxr(int warps, int ctas) { return coresident_regs(warps * ctas); }
@@ -320,14 +329,15 @@ static KernSet make_v5_set()
     constexpr int WXZ0 = 12;
     constexpr int CXZ = TWO_XZ ? 2 : (v5_smem_happly_xz<NX, NZ>(4, 2, WXZ0) <= SMEM_LIMIT) ? 4 : 2;
     constexpr int BXZ = (v5_smem_happly_xz<NX, NZ>(CXZ, 2, WXZ0) <= SMEM_LIMIT) ? 2 : 1;
-    constexpr int WXZ = TWO_XZ ? NZ / 4 : v5_warps((CXZ / 2) * NZ / 4, NX >= 32 ? 8 : 12);
+    constexpr int WXZ = TWO_XZ ? NZ / 4 : v5_warps((CXZ / 2) * NZ / 4, NX == 32 ? 8 : v5_wcap(NX));
     constexpr int WDY = imin(2 * (NY / 4) + 2 * (NZ / 4), imax(NY, NZ) >= 40 ? 8 : 12);
     constexpr int WDX = imin(2 * NZ / 4, NX >= 40 ? 8 : 12);
     static_assert(v5_smem_happly_yz<NY, NZ>(CYZ, BYZ, VST) <= SMEM_LIMIT, "yz plane too large");
     static_assert(v5_smem_happly_xz<NX, NZ>(CXZ, BXZ, WXZ) <= SMEM_LIMIT, "xz plane too large");
     KernSet k;
-    // register caps: 128 where a 12-warp CTA then leaves room for one update CTA per SM (overlap), else what fits
-    constexpr int RYZ = TWO_YZ ? v5_maxr(WYZ, 2) : v5_maxr(WYZ, 1), RXZ = TWO_XZ ? v5_maxr(WXZ, 2) : v5_maxr(WXZ, 1);
+    // register caps: the co-resident budget (room for the update CTA); a yz kernel of 10 or more warps takes the whole
+    // register file instead (at 144 registers its spills cost more than the overlap gains: 40^3, measured)
+    constexpr int RYZ = TWO_YZ ? v5_maxr(WYZ, 2) : (WYZ >= 10 ? v6_regs(WYZ) : v5_maxr(WYZ, 1)), RXZ = TWO_XZ ? v5_maxr(WXZ, 2) : v5_maxr(WXZ, 1);
     constexpr bool WST = !TWO_XZ && BXZ == 2 && v5_smem_happly_xz<NX, NZ>(CXZ, BXZ, WXZ, true) <= SMEM_LIMIT;
     k.h_yz = k5_happly_yz<NY, NZ, CYZ, BYZ, WYZ, VST, RYZ>; k.h_xz = k5_happly_xz<NX, NZ, CXZ, BXZ, WXZ, RXZ, WST>;
     k.cps_h[0] = TWO_YZ ? 2 : 1; k.cps_h[1] = TWO_XZ ? 2 : 1; k.tma_h[0] = k.tma_h[1] = 0;
@@ -346,11 +356,6 @@ static KernSet make_v5_set()
 // the yz-plane CTA's shared memory (edges <= 24) the yz kernel adds the pairing block, else (32^3, 2-spinor units) the
 // xz kernel does.  The ABM update is k7_update, co-resident with them; the density kernels and the starter's update
 // are those of plane5_kernels.cuh.
-static constexpr int v6_regs(int warps)
-{
-    const int r = (65536 / (warps * 32)) & ~7;
-    return r > 255 ? 255 : r;
-}
 template <int NX, int NY, int NZ>
 static KernSet make_v6_set()
 {
