@@ -40,8 +40,9 @@ CASES = {
     "both_12x8x16": (0, (12, 8, 16), 1.5, (20, 12), 10, None), # non-cubic, both species, Coulomb, ragged chunks
     "r2_6x10x12": (0, (6, 10, 12), 1.5, (7, 5), 6, None),      # sizes not divisible by 4 (R = 2 blocking)
     # 10 steps (3 starter + 7 ABM) on reduced-state versions of configs 1-4; 256 + 256 states on the
-    # config-1 lattice = two chunks per species at the default chunk size (the launch configuration bench.py times)
-    "c1_24c_256": (1, None, None, (256, 256), 10, None),
+    # config-1 lattice in three chunks per species (96 + 96 + 64) with the stream overlap on: the launch configuration
+    # bench.py times (full state groups in every CTA, double-buffered W, densities per group of 2 chunks)
+    "c1_24c_256": (1, None, None, (256, 256), 10, dict(chunk=96, dgroup=2, overlap=True)),
     # the multi-chunk pipeline: 7 + 4 chunks with ragged tails, double-buffered W / eta, update on the second stream,
     # density launches per group of 3 chunks (a species change inside a group)
     "c1_24c_pipeline": (1, None, None, (40, 24), 10, dict(chunk=6, dgroup=3, overlap=True)),
