@@ -126,6 +126,22 @@ struct RDFT<5> {                                   // spectral order b0, b1, e1,
         y[0] = a[0] + a[1] + a[3]; y[1] = A1 + B1; y[2] = A2 + B2; y[3] = A2 - B2; y[4] = A1 - B1;
     }
 };
+template <>
+struct RDFT<6> {                                   // spectral order b0, b1, e1, b2, e2, b3
+    static __device__ __forceinline__ void fwd(const double (&x)[6], double (&v)[6])
+    {
+        const double s03 = x[0] + x[3], d03 = x[0] - x[3], s14 = x[1] + x[4], d14 = x[1] - x[4], s25 = x[2] + x[5], d25 = x[2] - x[5];
+        v[0] = s03 + s14 + s25; v[1] = fma(0.5, d14 - d25, d03); v[2] = LISE_SIN60 * (d14 + d25);
+        v[3] = fma(-0.5, s14 + s25, s03); v[4] = LISE_SIN60 * (s14 - s25); v[5] = d03 - d14 + d25;
+    }
+    static __device__ __forceinline__ void inv(const double (&a)[6], double (&y)[6])
+    {
+        const double P = fma(-0.5, a[3], a[0]), Q = fma(0.5, a[1], -a[5]);
+        const double sp = LISE_SIN60 * (a[2] + a[4]), sm = LISE_SIN60 * (a[2] - a[4]);
+        y[0] = a[0] + a[1] + a[3] + a[5]; y[3] = a[0] - a[1] + a[3] - a[5];
+        y[1] = P + Q + sp; y[2] = P - Q + sm; y[4] = P - Q - sm; y[5] = P + Q - sp;
+    }
+};
 #define LISE_SQRT_HALF 0.70710678118654752440
 template <>
 struct RDFT<8> {                                   // spectral order b0, b1, e1, b2, e2, b3, e3, b4

@@ -49,6 +49,8 @@ CASES = {
     "c2_32c": (2, None, None, (64, 64), 10, None),
     "c3_24x24x64": (3, None, None, (64, 64), 10, None),
     "c4_40c": (4, None, None, (64, 64), 10, None),
+    # the paper's own fission box 24^2 x 48 (L1076): 48-point lines = 8 x 6, the size-6 real DFT of the DMMA line operator
+    "p_24x24x48": (3, (24, 24, 48), None, (12, 8), 5, None),
 }
 
 
