@@ -491,6 +491,77 @@ def test_free_two_mode_state_exact_phase():
     assert np.abs(got2[0, 0] - w2).max() / np.abs(w2).max() < 1e-8
 
 
+def test_static_scf_solution_is_stationary():
+    """SURVEY 8(c) "stationarity of a tiny static solution": a self-consistent Hartree-Fock state (pairing off,
+    Coulomb on, 2 neutrons + 2 protons on 6^3) is built HERE by dense diagonalisation of the single-particle h of
+    Eq. 12 (tests/dense_ref.py, Kronecker products of the closed-form Eq. 48 matrices) in the oracle's mean field,
+    iterated with linear density mixing.  With v_k = conj(phi_k) of the occupied orbitals (Eq. 11: the v sector
+    carries -h*) the oracle's time evolution must leave wavefunctions, densities and energy unchanged (Eqs. 80-81
+    remove the phase e^{+i eps t}): this ties densities -> mean field -> H psi -> stepper into one loop."""
+    from tests import dense_ref
+    shape, a = (6, 6, 6), 1.6
+    nxyz = int(np.prod(shape)); dV = a ** 3
+    par = ref.default_params(); par.g0_n = 0.0; par.g0_p = 0.0
+    c = ref.RefContext(*shape, a, 0.05, 2, 2, params=par)
+    x = np.meshgrid(*[(np.arange(n) - n / 2 + 0.5) * a for n in shape], indexing="ij")
+    g = np.exp(-sum(q * q for q in x) / (2 * 1.8 ** 2)); g /= math.sqrt(dV * (g * g).sum())
+
+    def states(orbs):                       # orbs: [2, 2 nxyz] spin-major spinors phi_k -> psi_k = (0, 0, conj phi_k)
+        psi = np.zeros((2, 4) + shape, complex)
+        for k in range(2):
+            psi[k, 2:] = np.conj(orbs[k]).reshape((2,) + shape)
+        return psi
+    orb0 = np.zeros((2, 2 * nxyz), complex)
+    orb0[0, :nxyz] = g.reshape(-1); orb0[1, nxyz:] = g.reshape(-1)
+    psi = [states(orb0), states(orb0)]
+    dens = [c.densities_of(p) for p in psi]
+    eps = [None, None]
+    for it in range(400):
+        pn, pp, _ = c.potentials_from(dens[0], dens[1])
+        for q, t in enumerate((pn, pp)):
+            pot = dict(U=t[0].reshape(-1), M=t[1].reshape(-1), W=[t[3 + i].reshape(-1) for i in range(3)],
+                       S=[t[6 + i].reshape(-1) for i in range(3)], A=[t[9 + i].reshape(-1) for i in range(3)])
+            h = dense_ref.dense_h(shape, a, pot)
+            assert np.abs(h - h.conj().T).max() < 1e-10
+            w, v = np.linalg.eigh(h)
+            eps[q] = w[:2]
+            psi[q] = states((v[:, :2] / math.sqrt(dV)).T)
+        new = [c.densities_of(p) for p in psi]
+        change = max(np.abs(n_ - d_).max() for n_, d_ in zip(new, dens))
+        dens = [0.5 * d_ + 0.5 * n_ for n_, d_ in zip(new, dens)]
+        if change < 1e-13:
+            break
+    assert change < 1e-13, (it, change)
+    assert eps[0][1] < 0.0 and eps[1][1] < 0.0                     # bound orbitals (a Kramers pair each)
+    assert abs(eps[0][0] - eps[0][1]) < 1e-8 and eps[1][0] > eps[0][0]   # Coulomb lifts the proton level
+    for q in (0, 1):
+        c.set_wavefunctions(q, psi[q])
+    o0 = c.observables(); d0 = [c.densities(q) for q in (0, 1)]
+    # H psi_k = -eps_k psi_k for the v-type states, to the accuracy of the self-consistency
+    for q in (0, 1):
+        hp = c.apply_h(q, psi[q]).reshape(psi[q].shape)
+        for k in range(2):
+            assert np.abs(hp[k] + eps[q][k] * psi[q][k]).max() < 1e-9 * abs(eps[q][k]) * np.abs(psi[q][k]).max() + 1e-11
+    c.step(8)                                                    # 3 starter + 5 ABM steps
+    for q in (0, 1):
+        got = c.get_wavefunctions(q)
+        assert np.abs(got - psi[q]).max() < 1e-11 * np.abs(psi[q]).max()          # measured 2e-14
+        d1 = c.densities(q)
+        assert np.abs(d1[0] - d0[q][0]).max() < 1e-12 * np.abs(d0[q][0]).max()
+    o1 = c.observables()
+    assert abs(o1["energy"] - o0["energy"]) < 1e-12 * abs(o0["energy"])
+    # without phase removal the same state rotates with e^{+i eps t / hbar c} (v sector of Eq. 11)
+    par.remove_phase = 0
+    c2 = ref.RefContext(*shape, a, 0.05, 2, 2, params=par)
+    for q in (0, 1):
+        c2.set_wavefunctions(q, psi[q])
+    c2.step(4)
+    t = 4 * 0.05
+    got = c2.get_wavefunctions(0)
+    want = psi[0][0] * np.exp(1j * eps[0][0] * t / par.hbarc)
+    assert np.abs(got[0] - want).max() < 1e-10 * np.abs(want).max()
+
+
 def test_stepper_is_the_scalar_linear_recurrence_of_eq78_to_roundoff():
     """SURVEY 8(c) "ABM linear recurrence": interaction and phase removal off, one plane-wave state: H psi = E psi
     with a constant E, so the whole stepper (3 starter steps = multiplication by the 4th-order series T4(z), Eq. 77,
