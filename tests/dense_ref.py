@@ -105,3 +105,43 @@ def table3(pot, lapM, shape):
         t[9 + i] = pot["A"][i].reshape(shape)
     t[12] = pot["Delta"].real.reshape(shape); t[13] = pot["Delta"].imag.reshape(shape)
     return t
+
+
+def scf_ground_state(c, shape, a, nocc=2, width=1.8, mix=0.5, tol=1e-13, maxit=400):
+    """Self-consistent Hartree-Fock state in the mean field of the oracle context `c` (pairing must be off): per species
+    the `nocc` lowest orbitals of the dense single-particle h (dense_h above) occupied as v_k = conj(phi_k), u_k = 0
+    (Eq. 11: the v sector carries -h*), iterated with linear mixing of the 14 density fields until they stop changing.
+    Returns (psi[2] as [nocc, 4, nx, ny, nz] complex, eps[2] single-particle energies, iterations, last change)."""
+    import math
+    nxyz = int(np.prod(shape)); dV = a ** 3
+    x = np.meshgrid(*[(np.arange(n) - n / 2 + 0.5) * a for n in shape], indexing="ij")
+    g = np.exp(-sum(q * q for q in x) / (2 * width ** 2)); g /= math.sqrt(dV * (g * g).sum())
+
+    def states(orbs):                       # [nocc, 2 nxyz] spin-major spinors phi_k -> psi_k = (0, 0, conj phi_k)
+        psi = np.zeros((nocc, 4) + tuple(shape), complex)
+        for k in range(nocc):
+            psi[k, 2:] = np.conj(orbs[k]).reshape((2,) + tuple(shape))
+        return psi
+    orb0 = np.zeros((nocc, 2 * nxyz), complex)
+    for k in range(nocc):
+        orb0[k, (k % 2) * nxyz:(k % 2 + 1) * nxyz] = g.reshape(-1) * (1.0 + 0.1 * (k // 2) * x[0].reshape(-1))
+    psi = [states(orb0), states(orb0)]
+    dens = [c.densities_of(p) for p in psi]
+    eps = [None, None]
+    change = None
+    for it in range(maxit):
+        pn, pp, _ = c.potentials_from(dens[0], dens[1])
+        for q, t in enumerate((pn, pp)):
+            pot = dict(U=t[0].reshape(-1), M=t[1].reshape(-1), W=[t[3 + i].reshape(-1) for i in range(3)],
+                       S=[t[6 + i].reshape(-1) for i in range(3)], A=[t[9 + i].reshape(-1) for i in range(3)])
+            h = dense_h(shape, a, pot)
+            assert np.abs(h - h.conj().T).max() < 1e-9
+            w, v = np.linalg.eigh(h)
+            eps[q] = w[:nocc]
+            psi[q] = states((v[:, :nocc] / math.sqrt(dV)).T)
+        new = [c.densities_of(p) for p in psi]
+        change = max(np.abs(n_ - d_).max() for n_, d_ in zip(new, dens))
+        dens = [(1.0 - mix) * d_ + mix * n_ for n_, d_ in zip(new, dens)]
+        if change < tol:
+            break
+    return psi, eps, it, change

@@ -171,3 +171,38 @@ def test_boost_external_fields_and_frames():
     for q in (0, 1):
         assert field_rel(gc.potentials(q).cpu().numpy(), oc.potentials(q)) < 1e-10
     gc.close(); oc.close()
+
+
+def test_static_solution_stays_stationary_on_the_gpu():
+    """A self-consistent Hartree-Fock state (built on the CPU by dense diagonalisation in the oracle's mean field,
+    tests/dense_ref.py; pairing off, Coulomb on, 2 + 2 particles on 8^3: the FFT H-apply kernels) is a fixed point of the
+    phase-removed evolution (Eqs. 80-81): after 3 starter + 7 ABM steps of the CUDA path wavefunctions, density and
+    energy are those of the input, and H psi_k = -eps_k psi_k for the occupied v-type states."""
+    from paper_2009_00745_b200 import lise
+    from tests import dense_ref
+    shape, a, dt = (8, 8, 8), 1.5, 0.05
+    po = ref.default_params(); po.g0_n = 0.0; po.g0_p = 0.0
+    oc = ref.RefContext(*shape, a, dt, 2, 2, params=po)
+    psi, eps, it, change = dense_ref.scf_ground_state(oc, shape, a)
+    assert change < 1e-13, (it, change)
+    pg = _copy_params(po, lise.default_params())
+    gc = lise.Lise(*shape, a, dt, 2, 2, params=pg)
+    dev = [torch.from_numpy(p).cuda() for p in psi]
+    for q in (0, 1):
+        gc.set_wavefunctions(q, dev[q])
+    o0 = gc.observables()
+    d0 = [gc.densities(q).cpu().numpy() for q in (0, 1)]
+    for q in (0, 1):
+        hp = gc.apply_h(q, dev[q]).cpu().numpy()
+        for k in range(2):
+            assert np.abs(hp[k] + eps[q][k] * psi[q][k]).max() < 1e-9 * abs(eps[q][k]) * np.abs(psi[q][k]).max() + 1e-11
+    gc.step(10)
+    o1 = gc.observables()
+    for q in (0, 1):
+        got = gc.get_wavefunctions(q).cpu().numpy()
+        assert np.abs(got - psi[q]).max() < 1e-11 * np.abs(psi[q]).max()
+        d1 = gc.densities(q).cpu().numpy()
+        assert np.abs(d1[0] - d0[q][0]).max() < 1e-12 * np.abs(d0[q][0]).max()
+    assert abs(o1["energy"] - o0["energy"]) < 1e-12 * abs(o0["energy"])
+    assert abs(o1["n_neutron"] - 2.0) < 1e-12 and abs(o1["n_proton"] - 2.0) < 1e-12
+    gc.close(); oc.close()

@@ -500,37 +500,9 @@ def test_static_scf_solution_is_stationary():
     remove the phase e^{+i eps t}): this ties densities -> mean field -> H psi -> stepper into one loop."""
     from tests import dense_ref
     shape, a = (6, 6, 6), 1.6
-    nxyz = int(np.prod(shape)); dV = a ** 3
     par = ref.default_params(); par.g0_n = 0.0; par.g0_p = 0.0
     c = ref.RefContext(*shape, a, 0.05, 2, 2, params=par)
-    x = np.meshgrid(*[(np.arange(n) - n / 2 + 0.5) * a for n in shape], indexing="ij")
-    g = np.exp(-sum(q * q for q in x) / (2 * 1.8 ** 2)); g /= math.sqrt(dV * (g * g).sum())
-
-    def states(orbs):                       # orbs: [2, 2 nxyz] spin-major spinors phi_k -> psi_k = (0, 0, conj phi_k)
-        psi = np.zeros((2, 4) + shape, complex)
-        for k in range(2):
-            psi[k, 2:] = np.conj(orbs[k]).reshape((2,) + shape)
-        return psi
-    orb0 = np.zeros((2, 2 * nxyz), complex)
-    orb0[0, :nxyz] = g.reshape(-1); orb0[1, nxyz:] = g.reshape(-1)
-    psi = [states(orb0), states(orb0)]
-    dens = [c.densities_of(p) for p in psi]
-    eps = [None, None]
-    for it in range(400):
-        pn, pp, _ = c.potentials_from(dens[0], dens[1])
-        for q, t in enumerate((pn, pp)):
-            pot = dict(U=t[0].reshape(-1), M=t[1].reshape(-1), W=[t[3 + i].reshape(-1) for i in range(3)],
-                       S=[t[6 + i].reshape(-1) for i in range(3)], A=[t[9 + i].reshape(-1) for i in range(3)])
-            h = dense_ref.dense_h(shape, a, pot)
-            assert np.abs(h - h.conj().T).max() < 1e-10
-            w, v = np.linalg.eigh(h)
-            eps[q] = w[:2]
-            psi[q] = states((v[:, :2] / math.sqrt(dV)).T)
-        new = [c.densities_of(p) for p in psi]
-        change = max(np.abs(n_ - d_).max() for n_, d_ in zip(new, dens))
-        dens = [0.5 * d_ + 0.5 * n_ for n_, d_ in zip(new, dens)]
-        if change < 1e-13:
-            break
+    psi, eps, it, change = dense_ref.scf_ground_state(c, shape, a)
     assert change < 1e-13, (it, change)
     assert eps[0][1] < 0.0 and eps[1][1] < 0.0                     # bound orbitals (a Kramers pair each)
     assert abs(eps[0][0] - eps[0][1]) < 1e-8 and eps[1][0] > eps[0][0]   # Coulomb lifts the proton level
