@@ -316,50 +316,54 @@ static constexpr int v5_warps(int tasks, int cap)
     for (int w = cap; w >= cap / 2; --w) if (tasks % w == 0) return w;
     return cap;
 }
-// one plane-owner CTA per SM, whole states per unit if shared memory allows
-template <int NX, int NY, int NZ>
+// one plane-owner CTA per SM, whole states per unit if shared memory allows.  HAPPLY = false: only the update and density
+// kernels (the FFT kernel sets bring their own H-apply kernels).
+template <int NX, int NY, int NZ, bool HAPPLY = true>
 static KernSet make_v5_set()
 {
-    constexpr bool TWO_YZ = false, TWO_XZ = false;
-    // yz: prefer whole states with prefetch, then 2-spinors with prefetch, then 2-spinors without
-    constexpr int CYZ = TWO_YZ ? 2 : (v5_smem_happly_yz<NY, NZ>(4, 2, false) <= SMEM_LIMIT) ? 4 : 2;
-    constexpr int BYZ = (v5_smem_happly_yz<NY, NZ>(CYZ, 2, false) <= SMEM_LIMIT) ? 2 : 1;
-    constexpr bool VST = !TWO_YZ && v5_smem_happly_yz<NY, NZ>(CYZ, BYZ, true) <= SMEM_LIMIT;
-    constexpr int WYZ = TWO_YZ ? imax(NY, NZ) / 4 : (CYZ / 2) * v5_wpp(CYZ / 2, imax(NY, NZ) / 4, imax(NY, NZ));
-    constexpr int WXZ0 = 12;
-    constexpr int CXZ = TWO_XZ ? 2 : (v5_smem_happly_xz<NX, NZ>(4, 2, WXZ0) <= SMEM_LIMIT) ? 4 : 2;
-    constexpr int BXZ = (v5_smem_happly_xz<NX, NZ>(CXZ, 2, WXZ0) <= SMEM_LIMIT) ? 2 : 1;
-    constexpr int WXZ = TWO_XZ ? NZ / 4 : v5_warps((CXZ / 2) * NZ / 4, NX == 32 ? 8 : v5_wcap(NX));
+    KernSet k;
+    k.h_yz = nullptr; k.h_xz = nullptr;
+    k.cps_h[0] = k.cps_h[1] = 1; k.tma_h[0] = k.tma_h[1] = 0;
+    k.thr_h[0] = k.thr_h[1] = 0; k.smem_h[0] = k.smem_h[1] = 0; k.ups_xz = 1;
+    if constexpr (HAPPLY) {
+        // yz: prefer whole states with prefetch, then 2-spinors with prefetch, then 2-spinors without
+        constexpr int CYZ = (v5_smem_happly_yz<NY, NZ>(4, 2, false) <= SMEM_LIMIT) ? 4 : 2;
+        constexpr int BYZ = (v5_smem_happly_yz<NY, NZ>(CYZ, 2, false) <= SMEM_LIMIT) ? 2 : 1;
+        constexpr bool VST = v5_smem_happly_yz<NY, NZ>(CYZ, BYZ, true) <= SMEM_LIMIT;
+        constexpr int WYZ = (CYZ / 2) * v5_wpp(CYZ / 2, imax(NY, NZ) / 4, imax(NY, NZ));
+        constexpr int WXZ0 = 12;
+        constexpr int CXZ = (v5_smem_happly_xz<NX, NZ>(4, 2, WXZ0) <= SMEM_LIMIT) ? 4 : 2;
+        constexpr int BXZ = (v5_smem_happly_xz<NX, NZ>(CXZ, 2, WXZ0) <= SMEM_LIMIT) ? 2 : 1;
+        constexpr int WXZ = v5_warps((CXZ / 2) * NZ / 4, NX == 32 ? 8 : v5_wcap(NX));
+        static_assert(v5_smem_happly_yz<NY, NZ>(CYZ, BYZ, VST) <= SMEM_LIMIT, "yz plane too large");
+        static_assert(v5_smem_happly_xz<NX, NZ>(CXZ, BXZ, WXZ) <= SMEM_LIMIT, "xz plane too large");
+        // register caps: the co-resident budget (room for the update CTA); a yz kernel of 10 or more warps takes the whole
+        // register file instead (at 144 registers its spills cost more than the overlap gains: 40^3, measured)
+        constexpr int RYZ = WYZ >= 10 ? v6_regs(WYZ) : v5_maxr(WYZ, 1), RXZ = v5_maxr(WXZ, 1);
+        constexpr bool WST = BXZ == 2 && v5_smem_happly_xz<NX, NZ>(CXZ, BXZ, WXZ, true) <= SMEM_LIMIT;
+        k.h_yz = k5_happly_yz<NY, NZ, CYZ, BYZ, WYZ, VST, RYZ>; k.h_xz = k5_happly_xz<NX, NZ, CXZ, BXZ, WXZ, RXZ, WST>;
+        k.thr_h[0] = 32 * WYZ; k.thr_h[1] = 32 * WXZ;
+        k.smem_h[0] = v5_smem_happly_yz<NY, NZ>(CYZ, BYZ, VST); k.smem_h[1] = v5_smem_happly_xz<NX, NZ>(CXZ, BXZ, WXZ, WST);
+        k.ups_xz = 4 / CXZ;
+    }
     constexpr int WDY = imin(2 * (NY / 4) + 2 * (NZ / 4), imax(NY, NZ) >= 40 ? 8 : 12);
     constexpr int WDX = imin(2 * NZ / 4, NX >= 40 ? 8 : 12);
-    static_assert(v5_smem_happly_yz<NY, NZ>(CYZ, BYZ, VST) <= SMEM_LIMIT, "yz plane too large");
-    static_assert(v5_smem_happly_xz<NX, NZ>(CXZ, BXZ, WXZ) <= SMEM_LIMIT, "xz plane too large");
-    KernSet k;
-    // register caps: the co-resident budget (room for the update CTA); a yz kernel of 10 or more warps takes the whole
-    // register file instead (at 144 registers its spills cost more than the overlap gains: 40^3, measured)
-    constexpr int RYZ = TWO_YZ ? v5_maxr(WYZ, 2) : (WYZ >= 10 ? v6_regs(WYZ) : v5_maxr(WYZ, 1)), RXZ = TWO_XZ ? v5_maxr(WXZ, 2) : v5_maxr(WXZ, 1);
-    constexpr bool WST = !TWO_XZ && BXZ == 2 && v5_smem_happly_xz<NX, NZ>(CXZ, BXZ, WXZ, true) <= SMEM_LIMIT;
-    k.h_yz = k5_happly_yz<NY, NZ, CYZ, BYZ, WYZ, VST, RYZ>; k.h_xz = k5_happly_xz<NX, NZ, CXZ, BXZ, WXZ, RXZ, WST>;
-    k.cps_h[0] = TWO_YZ ? 2 : 1; k.cps_h[1] = TWO_XZ ? 2 : 1; k.tma_h[0] = k.tma_h[1] = 0;
     k.u[0] = nullptr; k.u[1] = k5_update<1>; k.u[2] = k5_update<2>; k.u[3] = k5_update<3>;
     constexpr int SBY = v5_dens_sb<NY, NZ>(), SBX = v5_dens_sb<NX, NZ>();
     k.d_yz = k5_dens_yz<NY, NZ, WDY, SBY>; k.d_x = k5_dens_x<NX, NZ, WDX, SBX>;
     k.name = "dmma"; k.v5 = 1;
-    k.thr_h[0] = 32 * WYZ; k.thr_h[1] = 32 * WXZ; k.thr_u = LISE_UPD_THREADS; k.thr_d = 32 * WDX; k.thr_dyz = 32 * WDY;
-    k.smem_h[0] = v5_smem_happly_yz<NY, NZ>(CYZ, BYZ, VST); k.smem_h[1] = v5_smem_happly_xz<NX, NZ>(CXZ, BXZ, WXZ, WST);
+    k.thr_u = LISE_UPD_THREADS; k.thr_d = 32 * WDX; k.thr_dyz = 32 * WDY;
     k.smem_u = 0; k.smem_d = v5_smem_dens_x<NX, NZ>(SBX); k.smem_dyz = v5_smem_dens_yz<NY, NZ>(SBY);
-    k.ups_xz = 4 / CXZ;
     return k;
 }
 // ---- FFT-cost line operator (fft_plane_kernels.cuh): one real line per thread, generated real-input FFT codelets.
 // Lattices with every edge in {8, 12, 16, 20, 24, 32}.  Both H-apply kernels are the FFT ones; where a whole state fits
 // the yz-plane CTA's shared memory (edges <= 24) the yz kernel adds the pairing block, else (32^3, 2-spinor units) the
-// xz kernel does.  The ABM update is k7_update, co-resident with them; the density kernels and the starter's update
-// are those of plane5_kernels.cuh.
+// xz kernel does.  The ABM update and the density kernels are those of plane5_kernels.cuh.
 template <int NX, int NY, int NZ>
 static KernSet make_v6_set()
 {
-    KernSet k = make_v5_set<NX, NY, NZ>();                     // update and density kernels
+    KernSet k = make_v5_set<NX, NY, NZ, false>();              // update and density kernels
     constexpr int CYZ = (YZGeom<NY, NZ, 4>::SMEM <= SMEM_LIMIT) ? 4 : 2;
     typedef YZGeom<NY, NZ, CYZ> GY;
     typedef XZGeom<NX, NZ> GX;
@@ -378,12 +382,9 @@ static KernSet make_v6_set()
 #define LISE_FFT_SHAPES(X) \
     X(8, 8, 8) X(12, 12, 12) X(16, 16, 16) X(20, 20, 20) X(24, 24, 24) X(32, 32, 32) X(12, 8, 16) X(16, 12, 8) X(12, 12, 16)
 
-// The DMMA plane kernels are instantiated for these lattices (nx, ny, nz): every lattice of BASELINE.json's
-// configs, the paper's 24^2 x 48, and two small non-cubic test shapes; every edge a multiple of 4 and the
-// planes small enough for shared memory.  Anything else runs the generic DFMA kernels.
-#define LISE_MMA_SHAPES(X) \
-    X(8, 8, 8) X(12, 12, 12) X(16, 16, 16) X(20, 20, 20) X(24, 24, 24) X(32, 32, 32) X(40, 40, 40) \
-    X(24, 24, 48) X(24, 24, 64) X(12, 8, 16) X(16, 12, 8)
+// The DMMA H-apply kernels are instantiated for the lattices the FFT kernels do not cover: 40^3 (BASELINE.json config 4),
+// the paper's 24^2 x 48 and 24^2 x 64 (config 3).  Anything else runs the generic DFMA kernels.
+#define LISE_MMA_SHAPES(X) X(40, 40, 40) X(24, 24, 48) X(24, 24, 64)
 static bool pick_kernels(int nx, int ny, int nz, int R, KernSet* out)
 {
     {
