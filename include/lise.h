@@ -140,7 +140,8 @@ int lise_potentials(lise_ctx *ctx, int species, double *out14_dev);
 
 /* out = H * in for nstates states of `species` (Eq. 11 with mu = 0; h of Eq. 12 in the lattice form
  * of Eqs. 55, 56), H built from the densities of the context's current wavefunctions of both
- * species.  No eta subtraction, no 1/(i hbar).  in_dev and out_dev must not overlap. */
+ * species.  No eta subtraction, no 1/(i hbar).  in_dev and out_dev must not overlap.  nstates = 0 is a
+ * no-op (the pointers may then be null). */
 int lise_apply_h(lise_ctx *ctx, int species, const void *in_dev, void *out_dev, int nstates);
 
 /* Advances all states by nsteps time steps: the first 3 steps after lise_set_wavefunctions /

@@ -1114,7 +1114,8 @@ extern "C" int lise_potentials(lise_ctx* c, int q, double* out14_dev)
 
 extern "C" int lise_apply_h(lise_ctx* c, int q, const void* in_dev, void* out_dev, int nstates)
 {
-    if (!c || q < 0 || q > 1 || !in_dev || !out_dev || nstates < 0) return LISE_EINVAL;
+    if (!c || q < 0 || q > 1 || nstates < 0 || (nstates > 0 && (!in_dev || !out_dev))) return LISE_EINVAL;
+    if (nstates == 0) return LISE_OK;                // empty input: nothing to do, the pointers may be null
     TRY(need_both(c));
     TRY(ensure_potentials(c));
     const size_t slen = (size_t)4 * c->L.nxyz;

@@ -332,3 +332,33 @@ def test_edge_cases_and_errors():
     assert torch.equal(g.get_wavefunctions(0), psi)
     assert float(g.densities(1).abs().max()) == 0.0
     g.close()
+
+
+@pytest.mark.parametrize("nwf", [(1, 0), (0, 2), (1, 1)])
+def test_degenerate_state_counts(nwf):
+    """fewer states than state groups (most plane-owner CTAs, and one of the two unit pipelines of the xz kernel, have no
+    work), a single state, protons only (Coulomb on, no neutron at all): 3 starter + 3 ABM steps against the oracle."""
+    from paper_2009_00745_b200 import lise
+    cfg = dict(inputs.CONFIGS[0]); cfg["shape"] = (12, 12, 12)
+    psi = [inputs.make_species(cfg, q, nwf[q], seed=77 + q) for q in (0, 1)]
+    po = ref.default_params(); pg = lise.default_params()
+    po.coulomb = pg.coulomb = 1 if nwf[1] else 0
+    oc = ref.RefContext(*cfg["shape"], cfg["dx"], 0.05, *nwf, params=po)
+    gc = lise.Lise(*cfg["shape"], cfg["dx"], 0.05, *nwf, params=pg)
+    for q in (0, 1):
+        oc.set_wavefunctions(q, psi[q].numpy())
+        gc.set_wavefunctions(q, psi[q].cuda())
+    oc.step(6); gc.step(6)
+    for q in (0, 1):
+        if nwf[q] == 0:
+            assert float(gc.densities(q).abs().max()) == 0.0
+            continue
+        assert rel(gc.get_wavefunctions(q).cpu().numpy(), oc.get_wavefunctions(q)) < TOL_WF
+        assert field_rel(gc.densities(q).cpu().numpy(), oc.densities(q)) < TOL_DENS
+    eo, eg = oc.observables(), gc.observables()
+    assert abs(eg["energy"] - eo["energy"]) < TOL_E * abs(eo["energy"])
+    # H applied to zero states is a no-op
+    q = 0 if nwf[0] else 1
+    empty = torch.zeros((0, 4) + tuple(cfg["shape"]), dtype=torch.complex128, device="cuda")
+    assert gc.apply_h(q, empty).shape[0] == 0
+    gc.close(); oc.close()
