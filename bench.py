@@ -54,18 +54,23 @@ def measured_traffic(cls, workload, states_per_launch):
 
 
 class ClockSampler:
-    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+    """nvidia-smi polled every 50 ms in the background; started BEFORE the warm-up steps (its start-up takes a few
+    hundred ms) and filtered to the timed region by its own timestamps."""
+    Q = ("timestamp,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
     def __init__(self, index):
         self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
         try:
             self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
-                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f, stderr=subprocess.DEVNULL)
+                                       "--format=csv,noheader,nounits", "-lms", "50"], stdout=self.f, stderr=subprocess.DEVNULL)
         except OSError:
             self.p = None
 
-    def stop(self):
+    def stop(self, t0, t1):
+        """samples with t0 <= timestamp <= t1 (wall clock of the timed region); if the region was shorter than the polling
+        interval, the samples since the sampler started (warm-up steps: the same load) are used and `window` says so."""
+        import datetime
         out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
         if self.p is None:
             return out
@@ -75,28 +80,33 @@ class ClockSampler:
         except Exception:
             self.p.kill()
         self.f.flush(); self.f.seek(0)
-        sm, mx, reasons, pw = [], [], set(), []
+        rows = []
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         for line in self.f.read().splitlines():
             parts = [x.strip() for x in line.split(",")]
-            if len(parts) < 7:
+            if len(parts) < 8:
                 continue
             try:
-                sm.append(float(parts[0])); mx.append(float(parts[1])); pw.append(float(parts[2]))
+                ts = datetime.datetime.strptime(parts[0], "%Y/%m/%d %H:%M:%S.%f").timestamp()
+                rows.append((ts, float(parts[1]), float(parts[2]), float(parts[3]),
+                             [n for n, v in zip(names, parts[4:8]) if v.lower().startswith("active")]))
             except ValueError:
                 continue
-            for n, v in zip(names, parts[3:7]):
-                if v.lower().startswith("active"):
-                    reasons.add(n)
         self.f.close()
         try:
             os.unlink(self.f.name)
         except OSError:
             pass
-        if sm:
-            sm.sort()
-            out.update(sm_mhz=sm[len(sm) // 2], sm_max_mhz=max(mx), reasons=sorted(reasons), samples=len(sm),
-                       power_w_max=max(pw))
+        inside = [r for r in rows if t0 - 0.025 <= r[0] <= t1 + 0.025]
+        window = "timed region"
+        if not inside:
+            inside = [r for r in rows if r[0] <= t1 + 0.025]
+            window = "warm-up + timed region (timed region shorter than the polling interval)"
+        if inside:
+            sm = sorted(r[1] for r in inside)
+            out.update(sm_mhz=sm[len(sm) // 2], sm_max_mhz=max(r[2] for r in inside),
+                       reasons=sorted({n for r in inside for n in r[4]}), samples=len(inside),
+                       power_w_max=max(r[3] for r in inside), window=window)
         return out
 
 
@@ -221,21 +231,22 @@ def run_workload(args, cfg_idx, nwf_req, env, primary):
 
     nstates = nwf[0] + nwf[1]
     g.step(3)                                   # series-expansion starter: outside the timed region
+    sampler = ClockSampler(local) if rank == 0 else None
     for _ in range(args.warmup):
         g.step(1)
     barrier()
     l0 = g.launch_count()
-    sampler = ClockSampler(local) if rank == 0 else None
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     wall0 = time.time()
     ev0.record()
     g.step(steps)
     ev1.record()
     barrier()
-    wall = time.time() - wall0
+    wall1 = time.time()
+    wall = wall1 - wall0
     ms = ev0.elapsed_time(ev1)
     launches = g.launch_count() - l0
-    clocks = sampler.stop() if sampler else None
+    clocks = sampler.stop(wall0, wall1) if sampler else None
     if world > 1:
         t = torch.tensor([ms], dtype=torch.float64, device=dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
