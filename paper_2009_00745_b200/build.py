@@ -7,9 +7,10 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "liblise.so")
-SOURCES = ["lise.cu"]
-NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-shared"]
+# source -> extra flags; happly_yz_whole.cu: the whole-state FFT yz kernels are faster with ptxas' lower register-usage
+# level (fewer spills at their 168-register cap), every other kernel with the default (csrc/fft_plane_kernels.cuh)
+SOURCES = {"lise.cu": [], "happly_yz_whole.cu": ["-Xptxas", "--register-usage-level=3"]}
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC"]
 
 
 def _deps():
@@ -51,9 +52,22 @@ def build(force=False, verbose=False):
             _codelets()
             nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
             tmp = SO + f".tmp{os.getpid()}"
-            cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SOURCES
-            subprocess.run(cmd, check=True, cwd=CSRC)
-            os.replace(tmp, SO)
+            objs, procs = [], []
+            for src, extra in SOURCES.items():                # the translation units compile side by side
+                obj = os.path.join(CSRC, src[:-3] + f".tmp{os.getpid()}.o")
+                objs.append(obj)
+                cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-c", "-o", obj, src]
+                procs.append((cmd, subprocess.Popen(cmd, cwd=CSRC)))
+            try:
+                for cmd, p in procs:
+                    if p.wait() != 0:
+                        raise subprocess.CalledProcessError(p.returncode, cmd)
+                subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", tmp] + objs, check=True, cwd=CSRC)
+                os.replace(tmp, SO)
+            finally:
+                for o in objs:
+                    if os.path.exists(o):
+                        os.unlink(o)
         finally:
             fcntl.flock(lock, fcntl.LOCK_UN)
     return SO

@@ -546,3 +546,16 @@ __global__ void __maxnreg__(MAXR) k6_happly_xz(const __grid_constant__ HArgs a)
     if (leader && uprev >= 0) flush_eta(uprev, it - 1);
     tmem_free<G::TCOLS>(tbase, warp);
 }
+
+// every register of the SM for a CTA of `warps` warps that runs without a neighbour: the register file is per
+// sub-partition (16384 each), which ceil(warps / 4) warps share
+__host__ __device__ constexpr int fft_full_regs(int warps)
+{
+    const int r = (16384 / (((warps + 3) / 4) * 32)) & ~7;
+    return r > 255 ? 255 : r;
+}
+// The whole-state yz kernels (edges <= 24) live in their own translation unit, happly_yz_whole.cu, which build.py compiles
+// with ptxas --register-usage-level=3: at 24^3 that schedule spills 84 instead of 260 bytes and runs 18.7 instead of 20.4 ms
+// per step; every other kernel is faster at the default level (measured).
+typedef void (*K6Kern)(HArgs);
+template <int NY, int NZ> K6Kern k6_yz_whole();

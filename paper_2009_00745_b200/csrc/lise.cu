@@ -298,13 +298,7 @@ static constexpr int imax(int a, int b) { return a > b ? a : b; }
 static constexpr int v5_wcap(int nline) { return nline >= 48 ? 8 : nline >= 40 ? 10 : 12; }
 static constexpr int v5_wpp(int npair, int strips, int nline) { return imin(strips, v5_wcap(nline) / npair); }
 
-// every register of the SM for a CTA of `warps` warps that runs without a neighbour: the register file is per
-// sub-partition (16384 each), which ceil(warps / 4) warps share
-static constexpr int v6_regs(int warps)
-{
-    const int r = (16384 / (((warps + 3) / 4) * 32)) & ~7;
-    return r > 255 ? 255 : r;
-}
+static constexpr int v6_regs(int warps) { return fft_full_regs(warps); }
 // register cap of a DMMA H-apply kernel with `warps` warps and `ctas` CTAs per SM: what leaves room for the co-resident
 // update CTA (plane_common.cuh: coresident_regs, the budget is per SM sub-partition)
 static constexpr int v5_maxr(int warps, int ctas) { return coresident_regs(warps * ctas); }
@@ -372,7 +366,8 @@ static KernSet make_v6_set()
     constexpr bool WHOLE = (CYZ == 4);                         // the yz kernel sees whole states: it adds the pairing block
     // the yz kernel takes every register of the SM (its shared-memory pipe is the busiest unit: nothing gains from a
     // neighbour); the xz kernel leaves one warp of LISE_UPD_REGS registers per sub-partition to the update CTA
-    k.h_yz = k6_happly_yz<NY, NZ, CYZ, v6_regs(GY::NW), WHOLE>;
+    if constexpr (WHOLE) k.h_yz = k6_yz_whole<NY, NZ>();       // own translation unit (happly_yz_whole.cu)
+    else k.h_yz = k6_happly_yz<NY, NZ, CYZ, v6_regs(GY::NW), false>;
     k.cps_h[0] = 1; k.thr_h[0] = 32 * GY::NW; k.smem_h[0] = GY::SMEM; k.tma_h[0] = 1;
     k.h_xz = k6_happly_xz<NX, NZ, coresident_regs(GX::NW), !WHOLE>;
     k.cps_h[1] = 1; k.thr_h[1] = 32 * GX::NW; k.smem_h[1] = GX::SMEM; k.ups_xz = 1; k.tma_h[1] = 1;

@@ -465,7 +465,7 @@ __global__ void __launch_bounds__(LO::MAXT) k_dens_x(DArgs a)
 }
 
 // norms and sampled overlaps: out[(k*4 + t)] = dV <psi_k|psi_l>, l = k (t=0), k+1, k+2, k+nwf/2 (mod nwf)
-__global__ void k_overlaps(const cplx* __restrict__ Y, int nwf, int len, double dV, cplx* __restrict__ out)
+static __global__ void k_overlaps(const cplx* __restrict__ Y, int nwf, int len, double dV, cplx* __restrict__ out)
 {
     __shared__ double s_red[64];
     const int k = blockIdx.x, t = blockIdx.y;
