@@ -362,3 +362,20 @@ def test_degenerate_state_counts(nwf):
     empty = torch.zeros((0, 4) + tuple(cfg["shape"]), dtype=torch.complex128, device="cuda")
     assert gc.apply_h(q, empty).shape[0] == 0
     gc.close(); oc.close()
+
+
+def test_defects_of_a_non_orthonormal_set():
+    """norm and orthonormality defects of lise_observables on a set with a planted overlap sin(0.3) and a planted
+    norm 1.05^2: the closed-form values (the oracle is pinned to the same ones on the CPU)."""
+    import math
+    from paper_2009_00745_b200 import lise
+    from tests.test_oracle_pins import _defective_set
+    shape, dx, nwf, theta, scale = (8, 8, 8), 1.5, 6, 0.3, 1.05
+    psi = _defective_set(shape, dx, nwf, theta, scale)
+    g = lise.Lise(*shape, dx, 0.05, nwf, 0)
+    g.set_wavefunctions(0, torch.from_numpy(psi).cuda())
+    g.set_wavefunctions(1, torch.zeros((0, 4) + shape, dtype=torch.complex128, device="cuda"))
+    o = g.observables()
+    assert abs(o["norm_defect"] - (scale ** 2 - 1.0)) < 1e-12
+    assert abs(o["ortho_defect"] - math.sin(theta)) < 1e-12
+    g.close()

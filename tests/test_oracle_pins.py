@@ -491,6 +491,29 @@ def test_free_two_mode_state_exact_phase():
     assert np.abs(got2[0, 0] - w2).max() / np.abs(w2).max() < 1e-8
 
 
+def _defective_set(shape, dx, nwf, theta, scale):
+    """an orthonormal set with two planted defects: state 3 <- cos(theta) psi_3 + sin(theta) e^{0.7 i} psi_4 (overlap
+    <psi_3|psi_4> = sin(theta) e^{-0.7 i}, norm still 1) and state 1 <- scale psi_1 (norm scale^2, still orthogonal)."""
+    from paper_2009_00745_b200 import inputs
+    cfg = dict(inputs.CONFIGS[0]); cfg["shape"] = shape; cfg["dx"] = dx
+    psi = inputs.make_species(cfg, 0, nwf, seed=5).numpy().copy()
+    psi[3] = math.cos(theta) * psi[3] + math.sin(theta) * np.exp(0.7j) * psi[4]
+    psi[1] *= scale
+    return psi
+
+
+def test_norm_and_orthonormality_defects_have_their_closed_form_values():
+    """lise_observables' defects: max_k |<psi_k|psi_k> - 1| and the largest sampled |<psi_k|psi_l>|
+    (neighbours k + 1, k + 2 and k + nwf / 2) on a set with a planted overlap sin(theta) and a planted norm scale^2."""
+    shape, dx, nwf, theta, scale = (8, 8, 8), 1.5, 6, 0.3, 1.05
+    psi = _defective_set(shape, dx, nwf, theta, scale)
+    c = ref.RefContext(*shape, dx, 0.05, nwf, 0)
+    c.set_wavefunctions(0, psi)
+    o = c.observables()
+    assert abs(o["norm_defect"] - (scale ** 2 - 1.0)) < 1e-12
+    assert abs(o["ortho_defect"] - math.sin(theta)) < 1e-12
+
+
 def test_static_scf_solution_is_stationary():
     """SURVEY 8(c) "stationarity of a tiny static solution": a self-consistent Hartree-Fock state (pairing off,
     Coulomb on, 2 neutrons + 2 protons on 6^3) is built HERE by dense diagonalisation of the single-particle h of
