@@ -222,6 +222,40 @@ int lise_line_operator_cost(int n, int *inner_ops_host, int *outer_ops_host);
  * T_j = P_j e_j + Q_j b_j:  (C x)[r + H m] = sum_j cos(2 pi j m / R) S_j[r] + sin(2 pi j m / R) T_j[r]. */
 int lise_line_operator_tables(int n, double dx, double *tab_host, int cap, int *dims_host);
 
+/* Renormalisation without a context and without any allocation ("normalise every qpwf" against the
+ * slow loss of norm to round-off; the same operation lise_params.renormalize applies inside lise_step).
+ *
+ *   psi_k <- psi_k / sqrt(dV * sum_i |psi_k[i]|^2)      for k = 0 .. nstates-1, in place.
+ *
+ * For whom: code that holds the wavefunctions itself and cannot let a library allocate -- a run sized to fill the GPU
+ * (wavefunctions + multistep history take nearly all of HBM, typically out of the application's own memory pool, so a
+ * late cudaMalloc fails), or a time loop that cannot afford the device-wide stall of cudaMalloc / cudaFree.  Every
+ * other call here needs a context, and lise_create allocates.  This call performs no cudaMalloc, no cudaFree and calls
+ * no library routine that allocates; its per-state scratch (one double per state) is a fixed array inside liblise.so.
+ *
+ * Arguments: psi_dev DEVICE pointer, caller-owned, nstates * state_len interleaved complex128, state k at offset
+ *   k * state_len (for the block layout above state_len = 4 * nx * ny * nz); dV > 0 the volume element; cuda_stream a
+ *   cudaStream_t owned by the caller (NULL = legacy default stream).  The call only enqueues two kernels on that stream
+ *   and returns; it does not synchronise.  A state that is identically zero is left unchanged.  nstates = 0 is a no-op.
+ * Limit: nstates <= LISE_STATIC_MAX_STATES.  More is refused with LISE_EINVAL (nothing is enqueued) and
+ *   lise_static_last_error() says so; renormalise a longer array slice by slice.
+ * Cost: the array (LISE_STATIC_MAX_STATES doubles, 128 KB) occupies device memory on every GPU on which this library's
+ *   CUDA code is loaded, for the life of the process, used or not.
+ * First call on a device: it looks up the array's address on the current device (cudaGetSymbolAddress, which may have
+ *   to load the library's CUDA module there) and caches it; later calls on that device skip this.  Make that first call
+ *   during set-up, with the intended device current and before any stream capture is begun on the thread.
+ * Sharing: there is ONE array per device for all callers.  Each call overwrites entries 0 .. nstates-1 before it reads
+ *   them, so nothing has to be cleared between calls and whatever an earlier call left behind is never read.  Calls
+ *   enqueued on the same stream run one after the other and are safe.  Two calls that can run at the same time on one
+ *   device (different streams without an event between them, two host threads on different streams) race on the array
+ *   and give wrong norms: order them yourself.
+ * Errors: LISE_EINVAL (null psi_dev, negative nstates, state_len <= 0, dV not positive and finite, nstates over the
+ *   limit), LISE_ECUDA (address lookup or launch failed), LISE_EUNSUPPORTED (device ordinal >= 64).  The message of the
+ *   calling thread's last failure is lise_static_last_error() (HOST string owned by the library, "" after a success). */
+#define LISE_STATIC_MAX_STATES 16384
+int lise_renormalize_static(void *psi_dev, int nstates, long long state_len, double dV, void *cuda_stream);
+const char *lise_static_last_error(void);
+
 /* Number of kernel launches issued by this context so far (for bench.py's gpu_launches). */
 long lise_launch_count(const lise_ctx *ctx);
 /* Bytes of device memory held by the context. */

@@ -9,7 +9,8 @@ CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "liblise.so")
 # source -> extra flags; happly_yz_whole.cu: the whole-state FFT yz kernels are faster with ptxas' lower register-usage
 # level (fewer spills at their 168-register cap), every other kernel with the default (csrc/fft_plane_kernels.cuh)
-SOURCES = {"lise.cu": [], "happly_yz_whole.cu": ["-Xptxas", "--register-usage-level=3"]}
+# no_alloc.cu: the allocation-free entry point and its fixed device array live in one translation unit of their own
+SOURCES = {"lise.cu": [], "happly_yz_whole.cu": ["-Xptxas", "--register-usage-level=3"], "no_alloc.cu": []}
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC"]
 
 

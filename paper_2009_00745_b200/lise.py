@@ -51,7 +51,10 @@ EXPORTS = ["lise_default_params", "lise_create", "lise_destroy", "lise_set_param
            "lise_upload_wavefunctions", "lise_download_wavefunctions", "lise_set_reduce_hook",
            "lise_densities", "lise_potentials", "lise_apply_h", "lise_step", "lise_observables", "lise_observables_ext",
            "lise_set_time", "lise_boost", "lise_set_external_fields", "lise_set_frame",
-           "lise_profile", "lise_profile_read", "lise_measure_fp64_peak", "lise_set_density_group", "lise_line_operator", "lise_line_operator_cost", "lise_line_operator_tables", "lise_launch_count", "lise_device_bytes", "lise_strerror", "lise_last_error"]
+           "lise_profile", "lise_profile_read", "lise_measure_fp64_peak", "lise_set_density_group", "lise_line_operator", "lise_line_operator_cost", "lise_line_operator_tables", "lise_launch_count", "lise_device_bytes", "lise_strerror", "lise_last_error",
+           "lise_renormalize_static", "lise_static_last_error"]
+
+STATIC_MAX_STATES = 16384       # LISE_STATIC_MAX_STATES of include/lise.h
 
 
 REDUCE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_long)
@@ -115,6 +118,8 @@ def load():
     lib.lise_device_bytes.argtypes = [vp]; lib.lise_device_bytes.restype = C.c_longlong
     lib.lise_strerror.argtypes = [ip]; lib.lise_strerror.restype = C.c_char_p
     lib.lise_last_error.argtypes = [vp]; lib.lise_last_error.restype = C.c_char_p
+    lib.lise_renormalize_static.argtypes = [vp, ip, C.c_longlong, dp, vp]
+    lib.lise_static_last_error.argtypes = []; lib.lise_static_last_error.restype = C.c_char_p
     _lib = lib
     return lib
 
@@ -135,6 +140,27 @@ def measure_fp64_peak(seconds=1.0, stream=None):
     if rc != 0:
         raise RuntimeError(f"lise_measure_fp64_peak failed ({rc})")
     return tf.value
+
+
+def renormalize_static(psi, dV, stream=None):
+    """lise_renormalize_static: psi[k] <- psi[k] / sqrt(dV sum |psi[k]|^2) in place, for a contiguous CUDA complex128
+    tensor whose first axis counts the states (at most STATIC_MAX_STATES of them).  For callers that cannot let the
+    library allocate device memory (HBM already full of wavefunctions, or no cudaMalloc stall allowed in the time
+    loop): no context, and the per-state scratch is a fixed array inside liblise.so, shared by all calls on a device --
+    calls that may overlap on the GPU must be ordered by the caller.  Enqueued on `stream` (default: torch's current
+    stream on psi's device); does not synchronise."""
+    if not (psi.is_cuda and psi.dtype == torch.complex128 and psi.is_contiguous() and psi.dim() >= 2):
+        raise LiseError("renormalize_static expects a contiguous CUDA complex128 tensor [nstates, ...]")
+    lib = load()
+    nst = psi.shape[0]
+    slen = psi.numel() // nst if nst else 1
+    with torch.cuda.device(psi.device):
+        st = torch.cuda.current_stream(psi.device) if stream is None else stream
+        rc = lib.lise_renormalize_static(C.c_void_p(psi.data_ptr()), nst, slen, float(dV), C.c_void_p(st.cuda_stream))
+    if rc != 0:
+        raise LiseError(f"lise_renormalize_static failed: {lib.lise_strerror(rc).decode()} ({rc}) "
+                        f"{lib.lise_static_last_error().decode()}")
+    return psi
 
 
 def line_operator_cost(n):
