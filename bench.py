@@ -164,7 +164,7 @@ def executed_model(shape, line_op, lise):
         return 2.0 * (c[0] + c[1]) / n if c[0] else dmma_axis(n)
     pw = 50.0                                                      # pointwise + small transforms per point, component and axis
     fft_yz = line_op == "fft"
-    fft_xz = fft_yz and max(ny, nz) > 24                           # the xz kernel is the FFT one only on 2-spinor-unit lattices
+    fft_xz = fft_yz                                                # lise.cu make_v6_set: both H-apply kernels of an "fft" set run FFT lines
     ay = (fft_axis if fft_yz else dmma_axis)
     ax = (fft_axis if fft_xz else dmma_axis)
     return {
@@ -191,6 +191,11 @@ def run_workload(args, cfg_idx, nwf_req, env, primary):
     free, _ = torch.cuda.mem_get_info(dev)
     req = nwf
     nwf = lise.capacity_states(shape, free, nwf)                 # 7 state arrays must fit
+    if sum(nwf) == 0:                                             # (0, 0): not even 256 states per requested species fit
+        why = f"does not fit: {free / 2 ** 30:.1f} GiB free for {req[0]} + {req[1]} states of {S / 2 ** 20:.2f} MB x 7 arrays"
+        if primary:
+            raise SystemExit(f"bench.py: config {cfg_idx} {why}")
+        return {"skipped": why, "config": {"workload": f"config{cfg_idx}", "shape": list(shape), "nwf_requested": list(req)}} if rank == 0 else None
     tot = (nwf[0] * world, nwf[1] * world)                        # weak scaling: global counts
     seed = inputs.SEED0 + cfg_idx
     steps = args.steps if primary else max(2, min(args.steps, 3))
@@ -211,7 +216,7 @@ def run_workload(args, cfg_idx, nwf_req, env, primary):
     torch.cuda.empty_cache()
     g = lise.Lise(*shape, cfg["dx"], cfg["dt"], nwf[0], nwf[1])
     if world > 1:
-        sharding.attach(g, global_nwf=tot, coulomb=bool(cfg["coulomb"]))
+        sharding.attach(g, global_nwf=tot, coulomb=bool(cfg["coulomb"]))   # the workload's flag, the same on every rank
     if args.chunk:
         g.set_chunk(args.chunk)
     if args.dgroup:
@@ -390,7 +395,8 @@ def run_ours(args):
         for k in ("config", "clocks", "e2e", "gpu_launches", "roofline", "step_roofline", "wall_s_timed_region", "observables"):
             out[k] = res[k]
         # the other workload the target names (32^3), same invocation: its own clocks, rooflines, state counts
-        out["also"] = [{"metric": METRIC, "unit": UNIT, **{k: r[k] for k in ("value", "ms_per_step", "steps", "config", "clocks",
+        out["also"] = [r if "skipped" in r else
+                       {"metric": METRIC, "unit": UNIT, **{k: r[k] for k in ("value", "ms_per_step", "steps", "config", "clocks",
                         "gpu_launches", "roofline", "step_roofline", "observables")}} for r in also]
         if args.cpu_baseline and world == 1:
             from paper_2009_00745_b200 import inputs

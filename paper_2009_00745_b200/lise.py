@@ -191,13 +191,19 @@ def line_operator_tables(n, dx):
 def capacity_states(shape, free_bytes, requested, reserve_bytes=6 * 2 ** 30, multiple=256):
     """capacity rule of SURVEY 8(d) / Appendix C: the library keeps 7 state arrays of S = 64 Nxyz bytes per state
     (+ a chunk-sized H psi scratch and grid fields, covered by `reserve_bytes`).  Returns the (n, p) state counts that
-    fit `free_bytes` of device memory: `requested` if it fits, else the largest multiple of `multiple` per species."""
+    fit `free_bytes` of device memory: `requested` if it fits; else the capacity split in proportion to the request,
+    each species rounded down to a multiple of `multiple`; (0, 0) if that leaves a requested species without states
+    (the workload does not fit: the caller skips it instead of running into an out-of-memory error in lise_create)."""
     S = 64 * shape[0] * shape[1] * shape[2]
-    cap = int((free_bytes - reserve_bytes) // (7 * S))
-    if requested[0] + requested[1] <= cap:
-        return tuple(requested)
-    each = max(multiple, (cap // 2) // multiple * multiple)
-    return (min(requested[0], each), min(requested[1], each))
+    cap = max(0, int((free_bytes - reserve_bytes) // (7 * S)))
+    req = (int(requested[0]), int(requested[1]))
+    tot = req[0] + req[1]
+    if tot <= cap:
+        return req
+    fit = tuple(min(r, (cap * r // tot) // multiple * multiple) for r in req)
+    if any(r > 0 and f == 0 for r, f in zip(req, fit)):
+        return (0, 0)
+    return fit
 
 
 class LiseError(RuntimeError):

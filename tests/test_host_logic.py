@@ -55,3 +55,21 @@ def test_tables_reject_bad_arguments():
     assert lib.lise_line_operator_tables(16, 1.0, None, 0, dims) == 0
     buf = (C.c_double * 4)()
     assert lib.lise_line_operator_tables(16, 1.0, buf, 4, dims) != 0       # capacity too small
+
+
+def test_capacity_states_never_returns_more_than_fits():
+    """7 state arrays of 64 Nxyz bytes per state + a reserve must fit the free memory."""
+    from paper_2009_00745_b200 import lise
+    shape = (32, 32, 32); S = 64 * 32 ** 3; G = 2 ** 30
+    fits = lambda nwf, free, reserve: 7 * S * sum(nwf) + reserve <= free
+    assert lise.capacity_states(shape, 180 * G, (4096, 4096)) == (4096, 4096)          # the request fits: unchanged
+    got = lise.capacity_states(shape, 180 * G, (8192, 8192))                            # SURVEY finding 5: 16384 do not
+    assert got[0] == got[1] and got[0] % 256 == 0 and 0 < got[0] < 8192 and fits(got, 180 * G, 6 * G)
+    assert not fits((got[0] + 256, got[1] + 256), 180 * G, 6 * G)                       # and it is the largest such count
+    got = lise.capacity_states(shape, 100 * G, (12000, 0))                              # one species gets the whole device
+    assert got[1] == 0 and got[0] % 256 == 0 and got[0] > 6000 and fits(got, 100 * G, 6 * G)
+    got = lise.capacity_states(shape, 100 * G, (9000, 3000))                            # split follows the request
+    assert fits(got, 100 * G, 6 * G) and 2.5 < got[0] / got[1] < 3.5
+    assert lise.capacity_states(shape, 6 * G + 7 * S * 300, (4096, 4096)) == (0, 0)     # under 256 per species: nothing
+    assert lise.capacity_states(shape, 2 * G, (4096, 4096)) == (0, 0)                   # less free than the reserve
+    assert lise.capacity_states(shape, 2 * G, (0, 0)) == (0, 0)
