@@ -232,6 +232,7 @@ class Lise:
         self._stream_ptr = st.cuda_stream
         self._chk(self.lib.lise_set_stream(self._h, C.c_void_p(st.cuda_stream)), "lise_set_stream")
         self.params = default_params()
+        self.coulomb_requested = int(self.params.coulomb)   # what the caller asked for (sharding.attach decides from it)
         if nwf_p == 0:
             self.params.coulomb = 0            # lise_create's default for a context without proton states
         if params is not None:
@@ -264,6 +265,7 @@ class Lise:
 
     def set_params(self, params):
         self.params = params
+        self.coulomb_requested = int(params.coulomb)
         self._chk(self.lib.lise_set_params(self._h, C.byref(params)), "lise_set_params")
 
     def set_stream(self, stream):

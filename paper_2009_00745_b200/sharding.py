@@ -32,15 +32,38 @@ def allreduce_sum_(t, group=None):
     return t
 
 
-def attach(ctx, group=None, global_nwf=None, coulomb=True):
+def _allreduce_ints(vals, op, group=None):
+    """element-wise reduction over ranks of a few host integers (identity without an initialised process group)."""
+    if not (dist.is_available() and dist.is_initialized() and dist.get_world_size(group) > 1):
+        return list(vals)
+    t = torch.tensor(list(vals), dtype=torch.int64)
+    if dist.get_backend(group) == "nccl":
+        t = t.cuda()
+    dist.all_reduce(t, op=op, group=group)
+    return [int(v) for v in t.cpu()]
+
+
+def attach(ctx, group=None, global_nwf=None, coulomb=None):
     """make `ctx` (paper_2009_00745_b200.lise.Lise) sum its density accumulators over the ranks of `group`.
-    global_nwf = (neutron, proton) state counts over all ranks: Coulomb is decided from the GLOBAL proton count, so
-    that a rank that happens to own no proton state still computes the same potentials and energy as the others."""
+    Coulomb must be the same on every rank (lise.h: the flag alone decides), so it is decided here from what the caller
+    asked for and from the GLOBAL proton count: on iff requested and some rank holds proton states.  A rank that
+    happens to own no proton state (whose context therefore defaulted to Coulomb off) then still computes the same
+    potentials and energy as the others.  The request is ctx.coulomb_requested -- the flag of the params the context
+    was given, the library default otherwise; `coulomb` (True / False) overrides it, None keeps it.  The global proton
+    count is global_nwf[1] if given, else the sum over ranks of ctx.nwf[1].  Collective: every rank of `group` calls it."""
     if global_nwf is not None:
-        want = 1 if (global_nwf[1] > 0 and coulomb) else 0
-        if ctx.params.coulomb != want:
-            ctx.params.coulomb = want
-            ctx.set_params(ctx.params)
+        global_p = int(global_nwf[1])
+    else:
+        global_p = _allreduce_ints([ctx.nwf[1]], dist.ReduceOp.SUM, group)[0]
+    req = int(bool(ctx.coulomb_requested if coulomb is None else coulomb))
+    lo, hi = _allreduce_ints([req, -req], dist.ReduceOp.MIN, group)
+    if lo != -hi:
+        raise ValueError("sharding.attach: the ranks disagree about Coulomb (params.coulomb must be the same on every rank)")
+    want = 1 if (req and global_p > 0) else 0
+    if ctx.params.coulomb != want:
+        ctx.params.coulomb = want
+        ctx.set_params(ctx.params)
+        ctx.coulomb_requested = req          # set_params recorded the decided flag; keep the caller's request
     ctx.set_reduce_hook(lambda t: allreduce_sum_(t, group))
 
 

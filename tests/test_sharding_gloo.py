@@ -75,3 +75,62 @@ def test_density_allreduce_world2(tmp_path):
     assert np.abs(summed - full).max() <= 1e-12 * np.abs(full).max()
     obs = np.load(tmp_path / "obs.npy")
     assert obs[0] == pytest.approx(2e-3) and obs[1] == pytest.approx(2e-4)
+
+
+class _FakeCtx:
+    """stands in for lise.Lise in attach(): the fields and setters attach touches, no GPU."""
+
+    class _P:
+        def __init__(self, coulomb):
+            self.coulomb = coulomb
+
+    def __init__(self, nwf, requested):
+        self.nwf = nwf
+        self.coulomb_requested = requested
+        self.params = self._P(requested if nwf[1] > 0 else 0)       # Lise.__init__: no proton states -> Coulomb off
+        self.hook = None
+
+    def set_params(self, p):
+        self.params = p
+        self.coulomb_requested = int(p.coulomb)
+
+    def set_reduce_hook(self, fn):
+        self.hook = fn
+
+
+def _attach_worker(rank, world, port, out_dir):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        res = []
+        nwf = (4, 3) if rank == 0 else (4, 0)                       # rank 1 owns no proton state
+        for requested, override, global_nwf in ((1, None, None), (0, None, None), (1, None, (8, 3)), (0, True, None), (1, False, None)):
+            c = _FakeCtx(nwf, requested)
+            sharding.attach(c, global_nwf=global_nwf, coulomb=override)
+            res.append(c.params.coulomb)
+            assert c.hook is not None
+        c = _FakeCtx((4, 0), 1)                                     # no rank holds protons: off everywhere
+        sharding.attach(c)
+        res.append(c.params.coulomb)
+        c = _FakeCtx(nwf, 1 if rank == 0 else 0)                    # ranks disagree: refused on every rank
+        try:
+            sharding.attach(c)
+            res.append(-1)
+        except ValueError:
+            res.append(9)
+        np.save(os.path.join(out_dir, f"attach{rank}.npy"), np.array(res))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_attach_decides_coulomb_from_the_request_and_the_global_proton_count(tmp_path):
+    """a context configured with coulomb = 0 must stay off; a rank without proton states follows the others."""
+    mp.spawn(_attach_worker, args=(2, _free_port(), str(tmp_path)), nprocs=2, join=True)
+    want = [1, 0, 1, 1, 0, 0, 9]
+    for rank in (0, 1):
+        assert list(np.load(tmp_path / f"attach{rank}.npy")) == want, rank
+    # single process, no process group: the local counts decide
+    c = _FakeCtx((4, 0), 1); sharding.attach(c); assert c.params.coulomb == 0
+    c = _FakeCtx((4, 2), 0); sharding.attach(c); assert c.params.coulomb == 0 and c.coulomb_requested == 0
+    c = _FakeCtx((4, 2), 1); sharding.attach(c); assert c.params.coulomb == 1
