@@ -6,7 +6,7 @@
  * wavefunction (qpwf) on a periodic 3D lattice.  All arithmetic is IEEE fp64 (complex128) in
  * hand-written CUDA kernels for sm_100a; there is no CPU fallback and no cuFFT/cuBLAS on this path.
  * Citations are "PAPER.md:L<line>" of the paper text plus equation numbers; the adopted reading of
- * every garbled or ambiguous passage is listed in DESIGN.md (ledger B1..B27).
+ * every garbled or ambiguous passage is listed in DESIGN.md (ledger B1..B32).
  *
  * Conventions
  *   species     0 = neutrons, 1 = protons; nwf_p = 0 means this context holds no proton states: Coulomb then defaults
@@ -174,7 +174,10 @@ int lise_set_time(lise_ctx *ctx, double time, long step);
  * Re-accumulates the densities and restarts the multistep method (the next three steps use the starter). */
 int lise_boost(lise_ctx *ctx, int species, const double *chi_dev);
 /* External fields (Eq. 24): h_q -> h_q + U0 - (1/2) [Uvec . p + p . Uvec].  u0_dev: Nxyz doubles (MeV), uvec_dev:
- * 3 Nxyz doubles, component-major, in units of c; DEVICE pointers, copied into the context; NULL removes the field. */
+ * 3 Nxyz doubles, component-major, in units of c; DEVICE pointers, copied into the context; NULL removes the field.
+ * STATIC fields only: the copy made here serves every H evaluation until the next call -- within a step both H[y_n] (time t_n)
+ * and H[m] (time t_{n+1}), and both evaluations of a start-up step.  The paper's fields depend on time; calling
+ * this between lise_step(ctx, 1) calls approximates that with a step-wise constant field, i.e. to first order in dt only. */
 int lise_set_external_fields(lise_ctx *ctx, int species, const double *u0_dev, const double *uvec_dev);
 /* Moving and rotating frame (Eqs. 26, 36): h -> h - v_cm . p - omega . (l + s) for both species, l = (r - origin) x p;
  * v_cm_host in units of c, omega_host in c / fm, origin_host in fm (HOST pointers to 3 doubles; NULL = zero). */

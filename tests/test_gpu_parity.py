@@ -20,17 +20,22 @@ def rel(a, b):
 
 
 def field_rel(got, want):
-    """per-field max-norm relative error for [nfields, ...] arrays; fields that are identically ~0 in the
-    reference are compared on the scale of the largest field."""
+    """per-field max-norm relative error for [nfields, ...] arrays, each field on its OWN scale.  Only a field that is
+    zero in the reference -- identically, or to the oracle's own round-off (<= 1e-12 of the largest field: e.g. the
+    Laplacian of a constant effective mass, a sum of cancelling terms) -- is compared on the scale of the largest field.
+    A field that carries a signal between 1e-12 and 1e-9 of the array scale cannot be compared at the parity tolerance
+    on either scale (round-off of the large fields leaks into it): that is a flaw of the test input, and it fails here
+    instead of passing unnoticed."""
     scale = np.abs(want).max()
     out = []
     for f in range(want.shape[0]):
         s = np.abs(want[f]).max()
-        small = not (s > 1e-9 * scale)
-        out.append(np.abs(got[f] - want[f]).max() / (scale if small else s))
-        if small and s > 0.0:        # a row that is merely small (not identically zero): make it visible in the log
-            print(f"field_rel: row {f} max {s:.3e} is below 1e-9 of the array scale {scale:.3e}; "
-                  f"error on its own scale {np.abs(got[f] - want[f]).max() / s:.3e}")
+        if s <= 1e-12 * scale:
+            out.append(np.abs(got[f] - want[f]).max() / scale if scale > 0.0 else np.abs(got[f]).max())
+            continue
+        assert s > 1e-9 * scale, (f"field_rel: row {f} has max {s:.3e}, between 1e-12 and 1e-9 of the array scale {scale:.3e}: "
+                                  f"too small to compare; error on its own scale {np.abs(got[f] - want[f]).max() / s:.3e}")
+        out.append(np.abs(got[f] - want[f]).max() / s)
     return max(out)
 
 
@@ -152,7 +157,7 @@ def test_full_size_single_evaluation_in_the_bench_launch_configuration(idx):
     shape = tuple(cfg["shape"])
     S = 64 * int(np.prod(shape))
     nwf = lise.capacity_states(shape, free, tuple(cfg["nwf"]))
-    if free < 7 * S * sum(nwf) + 6 * 2 ** 30 or (idx == 1 and nwf != tuple(cfg["nwf"])):
+    if sum(nwf) == 0 or free < 7 * S * sum(nwf) + 6 * 2 ** 30 or (idx == 1 and nwf != tuple(cfg["nwf"])):
         pytest.skip("not enough free device memory for the full-size workload")
     seed = inputs.SEED0 + idx
     # inputs first (the generator's workspace and the context's 7 arrays do not fit side by side at capacity)

@@ -135,6 +135,45 @@ def test_spherical_cutoff_geff_equals_the_regulated_integral():
     assert ref.inv_geff_spherical(g0, M, 100.0, -8.0, 60.0) == 0.0
 
 
+def test_lattice_cutoff_geff_counter_term_is_the_momentum_integral_over_the_brillouin_cube():
+    """Eq. 21, pinned without K and without retyping its prefactor: the term subtracted from 1/g0 is
+    the free-particle pairing loop regulated by the lattice's own momentum cutoff, every |k_i| <= pi/a:
+        1/g0 - 1/g_eff = int_{|k_i| <= pi/a} d^3k / (2 pi)^3  1 / (2 M k^2),    M = hbar^2 / 2 m*(r)
+    (the same integral that Eq. 20 cuts off spherically).  With k = (pi/a) x this is I / (16 pi^2 a M) with
+    I = int_{[-1,1]^3} d^3x / |x|^2.  Radially, int_0^R dr r^2 / r^2 = R(direction), and over the pyramid under the face
+    z = 1, with (u, v, 1) the point where the ray leaves the cube, dOmega = du dv / (1+u^2+v^2)^(3/2) and R = sqrt(1+u^2+v^2):
+        I = 6 int_{-1}^{1} int_{-1}^{1} du dv / (1 + u^2 + v^2)    -- a smooth 2-D quadrature, done here.
+    The oracle side is read off its outputs: Delta = -g_eff kappa (Eq. 19), so 1/g0 - 1/g_eff = 1/g0 + kappa/Delta.  A wrong
+    factor in the m* <-> M conversion, in the powers of pi or in a fails this."""
+    import scipy.integrate
+    I2, err = scipy.integrate.dblquad(lambda v, u: 1.0 / (1.0 + u * u + v * v), -1.0, 1.0, -1.0, 1.0, epsabs=1e-13, epsrel=1e-13)
+    I = 6.0 * I2
+    # coarse brute-force guard of the reduction itself: midpoint rule of 1/|x|^2 on the cube (the singularity is integrable;
+    # the rule converges like h), compared at 1e-2
+    n = 96
+    x = (np.arange(n) + 0.5) / n
+    X, Y, Z = np.meshgrid(x, x, x, indexing="ij")
+    brute = 8.0 * (1.0 / (X * X + Y * Y + Z * Z)).sum() / n ** 3
+    assert abs(brute - I) < 1e-2 * I, (brute, I)
+    shape, a = (10, 10, 12), 1.25
+    rng = np.random.default_rng(21)
+    for a in (1.25, 1.0):
+        par = ref.default_params(); par.coulomb = 0                    # alpha_pair = 0: g0(r) = g0 (Eq. 8)
+        c = ref.RefContext(*shape, a, 0.05, 1, 1, params=par)
+        dn, dp = _smooth_densities(shape, a, rng)
+        pots = c.potentials_from(dn, dp)
+        for q, d, g0 in ((0, dn, par.g0_n), (1, dp, par.g0_p)):
+            M = pots[q][1]
+            assert M.max() - M.min() > 0.5                             # m*(r) really varies over the box
+            kappa = d[12] + 1j * d[13]
+            delta = pots[q][12] + 1j * pots[q][13]
+            counter = 1.0 / g0 + kappa / delta
+            want = I / (16.0 * math.pi ** 2 * a * M)
+            assert np.abs(counter.imag).max() < 1e-12 * np.abs(want).max()
+            assert np.abs(counter.real - want).max() < 1e-8 * np.abs(want).max(), (q, a)
+        c.close()
+
+
 def _fd_du(c, dn, dp, q, delta, eps=1e-5):
     """(E[n_q + eps delta] - E[n_q - eps delta]) / 2 eps at fixed other fields, and dV sum U_q delta."""
     d = [dn, dp]
