@@ -198,7 +198,7 @@ def run_workload(args, cfg_idx, nwf_req, env, primary):
         return {"skipped": why, "config": {"workload": f"config{cfg_idx}", "shape": list(shape), "nwf_requested": list(req)}} if rank == 0 else None
     tot = (nwf[0] * world, nwf[1] * world)                        # weak scaling: global counts
     seed = inputs.SEED0 + cfg_idx
-    steps = args.steps if primary else max(2, min(args.steps, 3))
+    steps = args.steps                                            # every workload of the line gets the full --steps
 
     # inputs first, parked in pinned host memory: the generator's workspace and the context's 7 arrays do not fit side
     # by side at capacity; the host copies are also the end-to-end leg's mirror
@@ -368,17 +368,28 @@ def run_ours(args):
     import torch.distributed as dist
     from paper_2009_00745_b200 import lise
 
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # `python bench.py --gpus N` without a launcher: re-run this command line under torch.distributed.run, one rank
+        # per GPU, so that a scaling run can never silently measure one GPU and label it N
+        import socket
+        with socket.socket() as so:
+            so.bind(("127.0.0.1", 0))
+            port = so.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        sys.stdout.flush()
+        os.execv(sys.executable, cmd)
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.gpus != world:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but the launcher started WORLD_SIZE={world} ranks")
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback (use --impl reference for the oracle)")
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
-    if args.gpus != world and rank == 0:
-        print(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}; using {world}", file=sys.stderr)
     env = dict(world=world, rank=rank, local=local, dev=dev, fp64_tf=lise.measure_fp64_peak(1.5) if rank == 0 else 0.0)
     res = run_workload(args, args.config, args.nwf, env, primary=True)
     also = []
