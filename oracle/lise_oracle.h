@@ -107,6 +107,12 @@ int  lise_ref_set_time(lise_ref_ctx *c, double time, long step);
 int  lise_ref_boost(lise_ref_ctx *c, int species, const double *chi);
 /* Eq. 24: h_q -> h_q + U0 - (1/2) [Uvec . p + p . Uvec]; u0: Nxyz doubles (MeV), uvec: 3 Nxyz doubles (units of c); NULL = none */
 int  lise_ref_set_external_fields(lise_ref_ctx *c, int species, const double *u0, const double *uvec);
+/* L232: the fields of Eq. 24 depend on time.  The stored profiles are multiplied by f_now wherever H is built from y_n
+ * (time t_n: first evaluation of Eq. 78, Eq. 75, potentials / apply_h / observables of the current state), by f_next in
+ * the evaluation on the modifier (time t_{n+1}, Eq. 78c), and by (f_now + f_next) / 2 in the starter's H_cor, whose
+ * densities are averaged the same way (Eq. 76; reading B33).  Default 1, 1.  Frame terms are not scaled.
+ * The pair holds until it is set again: a driven run calls this before every single step. */
+int  lise_ref_set_external_amplitudes(lise_ref_ctx *c, double f_now, double f_next);
 /* Eqs. 26, 36: h -> h - v_cm . p - omega . (l + s), l = (r - origin) x p; v_cm in units of c, omega in c / fm, origin in fm */
 int  lise_ref_set_frame(lise_ref_ctx *c, const double *v_cm, const double *omega, const double *origin);
 /* Eqs. 37-41 of the current wavefunctions / of externally supplied Table-2 densities and Table-3 potentials */

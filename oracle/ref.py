@@ -70,6 +70,7 @@ def lib():
         _lib.lise_ref_inv_geff_spherical.restype = C.c_double
         _lib.lise_ref_inv_geff_spherical.argtypes = [C.c_double] * 5
         _lib.lise_ref_set_time.argtypes = [C.c_void_p, C.c_double, C.c_long]
+        _lib.lise_ref_set_external_amplitudes.argtypes = [C.c_void_p, C.c_double, C.c_double]
         _lib.lise_ref_abm_predict.argtypes = [C.c_long, C.c_double] + [C.c_void_p] * 9
         _lib.lise_ref_abm_correct.argtypes = [C.c_long, C.c_double] + [C.c_void_p] * 9
     return _lib
@@ -167,6 +168,9 @@ class RefContext:
         assert b is None or b.size == 3 * self.nxyz
         _chk(lib().lise_ref_set_external_fields(self._h, q, None if a is None else _p(a), None if b is None else _p(b)),
              "set_external_fields")
+
+    def set_external_amplitudes(self, f_now, f_next):
+        _chk(lib().lise_ref_set_external_amplitudes(self._h, float(f_now), float(f_next)), "set_external_amplitudes")
 
     def set_frame(self, v_cm=(0, 0, 0), omega=(0, 0, 0), origin=(0, 0, 0)):
         arrs = [np.ascontiguousarray(x, dtype=np.float64) for x in (v_cm, omega, origin)]

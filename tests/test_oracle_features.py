@@ -345,3 +345,67 @@ def test_h_with_external_terms_is_hermitian_and_energy_of_external_terms():
     assert abs(e_ext - want) < 1e-10 * max(abs(want), 1.0)
     assert np.abs(pots_with[0] - c.potentials(0)[0] - u0).max() < 1e-12
     c.close()
+
+
+def test_driven_free_state_follows_the_closed_form_phase_to_fourth_order():
+    """PAPER.md:L232 (Eq. 24 with U(r, t)): a uniform field U0 f(t) on the free two-mode state u_up = A e^{ik1.r},
+    v_up = B e^{ik2.r} (no phase removal) gives u(t) = u(0) exp(-i [E1 t + U0 F(t)] / hbar c) and
+    v(t) = v(0) exp(+i [E2 t + U0 F(t)] / hbar c), F = int_0^t f.  With the amplitude pair (f(t_n), f(t_{n+1})) supplied
+    before every step and an exact multistep history, the ABM error falls by >= 2^4 when dt is halved; with the starter
+    it falls like the starter's own third order; a field frozen at t_n during the step is only first order."""
+    shape, a = (8, 6, 4), 1.25
+    par = _free_params(); par.remove_phase = 0
+    x = np.meshgrid(*[np.arange(n) * a for n in shape], indexing="ij")
+    Ls = [n * a for n in shape]
+    k1 = np.array([2 * np.pi * 1 / Ls[0], 2 * np.pi * -1 / Ls[1], 0.0])
+    k2 = np.array([2 * np.pi * -1 / Ls[0], 0.0, 2 * np.pi * 1 / Ls[2]])
+    V = np.prod(Ls)
+    pw = lambda q: np.exp(1j * sum(qi * xi for qi, xi in zip(q, x)))
+    psi0 = np.zeros((1, 4) + shape, complex)
+    psi0[0, 0] = 0.8 / math.sqrt(V) * pw(k1); psi0[0, 2] = 0.6 / math.sqrt(V) * pw(k2)
+    E1, E2 = par.hbar2_2m * k1 @ k1, par.hbar2_2m * k2 @ k2
+    U0, w = 40.0, 0.9                                   # MeV; f(t) = cos(w t) + 0.3 t, F(t) = sin(w t) / w + 0.15 t^2
+    f = lambda t: math.cos(w * t) + 0.3 * t
+    F = lambda t: math.sin(w * t) / w + 0.15 * t * t
+    hc = par.hbarc
+
+    def exact(t):
+        y = np.zeros_like(psi0)
+        y[0, 0] = psi0[0, 0] * np.exp(-1j * (E1 * t + U0 * F(t)) / hc)
+        y[0, 2] = psi0[0, 2] * np.exp(+1j * (E2 * t + U0 * F(t)) / hc)
+        return y
+
+    def rhs(t):                                         # dy/dt of the exact solution
+        y = exact(t); g = np.zeros_like(y)
+        g[0, 0] = -1j * (E1 + U0 * f(t)) / hc * y[0, 0]
+        g[0, 2] = +1j * (E2 + U0 * f(t)) / hc * y[0, 2]
+        return g
+
+    def run(dt, T, history, frozen=False):
+        c = ref.RefContext(*shape, a, dt, 1, 0, params=par)
+        c.set_external_fields(0, u0=np.full(shape, U0))
+        c.set_wavefunctions(0, exact(0.0))
+        n = int(round(T / dt))
+        if history:                                     # exact y_{-1}, f_{-1..-3}, e_0 = 0: the ABM formulas alone
+            c.set_history(0, exact(-dt), rhs(-dt), rhs(-2 * dt), rhs(-3 * dt), np.zeros_like(psi0))
+        for i in range(n):
+            t = i * dt
+            c.set_external_amplitudes(f(t), f(t) if frozen else f(t + dt))
+            c.step(1)
+        got = c.get_wavefunctions(0)
+        c.close()
+        return np.abs(got - exact(n * dt)).max() / np.abs(psi0).max()
+
+    T = 1.6
+    e1, e2 = run(0.2, T, True), run(0.1, T, True)
+    assert e2 < 2e-6 and e1 / e2 > 16.0, (e1, e2)                   # fourth order or better
+    s1, s2 = run(0.2, T, False), run(0.1, T, False)
+    assert 5.0 < s1 / s2 < 20.0 and s2 < 1e-4, (s1, s2)             # the starter's third order (SURVEY 8(c))
+    z1, z2 = run(0.2, T, True, frozen=True), run(0.1, T, True, frozen=True)
+    assert 1.6 < z1 / z2 < 2.6 and z2 > 100 * e2, (z1, z2)          # what a per-step snapshot gives: first order
+    # amplitudes (1, 1) are the static field of lise_ref_set_external_fields
+    c = ref.RefContext(*shape, a, 0.05, 1, 0, params=par)
+    c.set_external_fields(0, u0=np.full(shape, U0)); c.set_wavefunctions(0, psi0); c.step(4)
+    want = psi0[0, 0] * np.exp(-1j * (E1 + U0) * 0.2 / hc)
+    assert np.abs(c.get_wavefunctions(0)[0, 0] - want).max() / np.abs(want).max() < 1e-8
+    c.close()
