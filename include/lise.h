@@ -21,7 +21,8 @@
  *   ordering    calls enqueue work on the context's stream and return without synchronising, except
  *               lise_observables (synchronises, writes host memory) and lise_create / lise_destroy.
  *   errors      every call returns LISE_OK (0) or a negative LISE_E* code; nothing throws or aborts.
- *               lise_last_error(ctx) gives a human-readable message for the last failure.
+ *               lise_last_error(ctx) gives a human-readable message for the last failure (ctx = NULL: for the
+ *               calling thread's last failed lise_create).  The library prints nothing.
  *   units       MeV, fm, fm/c.
  */
 #ifndef LISE_H
@@ -97,6 +98,15 @@ int lise_default_params(lise_params *p);
  * code holds 11, Eq. 83) plus a chunk-sized H psi scratch and grid fields.  Uses the current CUDA
  * device and the legacy default stream until lise_set_stream is called. */
 int lise_create(int nx, int ny, int nz, double dx, double dt, int nwf_n, int nwf_p, lise_ctx **out);
+/* lise_create with the line operator of the H-apply kernels chosen by the caller (for A/B checks of one kernel family
+ * against another, or as a way out if one misbehaves on some driver): line_operator (HOST string) = "fft", "dmma",
+ * "dense", or NULL / "auto" for lise_create's choice (see lise_line_operator below).  "dense" exists for every even
+ * lattice; "fft" and "dmma" only for the lattices they were instantiated for, otherwise LISE_EUNSUPPORTED; an unknown
+ * name is LISE_EINVAL.  All of them apply the same operator (Eqs. 48-50) and agree to round-off.  The automatic choice
+ * falls back to "dense" by itself when the driver lacks cuTensorMapEncodeTiled, which the "fft" kernels need.
+ * After a failed creation (either call) lise_last_error(NULL) returns the calling thread's message. */
+int lise_create_with_line_operator(int nx, int ny, int nz, double dx, double dt, int nwf_n, int nwf_p,
+                                   const char *line_operator, lise_ctx **out);
 void lise_destroy(lise_ctx *ctx);
 
 int lise_set_params(lise_ctx *ctx, const lise_params *p);
@@ -175,10 +185,17 @@ int lise_set_time(lise_ctx *ctx, double time, long step);
 int lise_boost(lise_ctx *ctx, int species, const double *chi_dev);
 /* External fields (Eq. 24): h_q -> h_q + U0 - (1/2) [Uvec . p + p . Uvec].  u0_dev: Nxyz doubles (MeV), uvec_dev:
  * 3 Nxyz doubles, component-major, in units of c; DEVICE pointers, copied into the context; NULL removes the field.
- * STATIC fields only: the copy made here serves every H evaluation until the next call -- within a step both H[y_n] (time t_n)
- * and H[m] (time t_{n+1}), and both evaluations of a start-up step.  The paper's fields depend on time; calling
- * this between lise_step(ctx, 1) calls approximates that with a step-wise constant field, i.e. to first order in dt only. */
+ * The copy made here is a spatial PROFILE; its time dependence (U(r,t), Uvec(r,t)) is the amplitude pair below.
+ * Replacing the profile between steps instead would freeze the field during each step: first order in dt only. */
 int lise_set_external_fields(lise_ctx *ctx, int species, const double *u0_dev, const double *uvec_dev);
+/* Time-dependent external fields: U0(r, t) = f(t) U0(r), Uvec(r, t) = f(t) Uvec(r) for both species, with f_now = f(t_n) and
+ * f_next = f(t_n + dt) supplied by the caller.  f_now multiplies the profiles wherever H is built from the current
+ * wavefunctions y_n (first evaluation of Eq. 78, Eq. 75, lise_potentials, lise_apply_h, e_ext); f_next in the evaluation on the
+ * modifier, which approximates y(t_{n+1}) (Eq. 78c); the start-up steps' corrector Hamiltonian, built from averaged
+ * densities (Eq. 76), takes (f_now + f_next) / 2 (reading B33).  Default 1, 1 = a static field.  The pair holds
+ * until it is set again, so a driven run calls this before every lise_step(ctx, 1); the frame terms are not scaled.
+ * The ABM steps then keep their order (the oracle pin shows >= 4th order on a driven free state).  Non-finite: LISE_EINVAL. */
+int lise_set_external_amplitudes(lise_ctx *ctx, double f_now, double f_next);
 /* Moving and rotating frame (Eqs. 26, 36): h -> h - v_cm . p - omega . (l + s) for both species, l = (r - origin) x p;
  * v_cm_host in units of c, omega_host in c / fm, origin_host in fm (HOST pointers to 3 doubles; NULL = zero). */
 int lise_set_frame(lise_ctx *ctx, const double *v_cm_host, const double *omega_host, const double *origin_host);

@@ -15,7 +15,7 @@ struct PhysConst {
     int coulomb, rearr, functional, cutoff;
 };
 // external fields of Eq. 24 per species (device pointers, NULL = none): scalar U0 [Nxyz], vector Uvec [3][Nxyz]
-struct ExtFields { const double* u0[2]; const double* uvec[2]; };
+struct ExtFields { const double* u0[2]; const double* uvec[2]; double amp; };   // amp: amplitude f(t) on both profiles
 
 // acc[f][r] = sum_g part[g][f][r] in fixed order (deterministic)
 __global__ void k_reduce_partials(const double* __restrict__ part, int G, size_t n, double* __restrict__ acc)
@@ -113,12 +113,12 @@ __device__ __forceinline__ double inv_geff_eq20(double g0r, double M, double U, 
 
 // component i of the vector field of the momentum-coupled external terms at lattice point r:
 // Uvec_ext + v_cm + omega x (r - origin)  (Eqs. 24, 26, 36; x_i = i a, Eq. 43)
-__device__ __forceinline__ double frame_uvec(const Lattice& L, const PhysConst& pc, const double* uvec, int i, int r)
+__device__ __forceinline__ double frame_uvec(const Lattice& L, const PhysConst& pc, const double* uvec, double amp, int i, int r)
 {
     const int iz = r % L.nz, iy = (r / L.nz) % L.ny, ix = r / (L.nz * L.ny);
     const double rr[3] = {ix * L.dx - pc.origin[0], iy * L.dx - pc.origin[1], iz * L.dx - pc.origin[2]};
     const int j1 = (i + 1) % 3, j2 = (i + 2) % 3;
-    return (uvec ? uvec[(size_t)i * L.nxyz + r] : 0.0) + pc.vcm[i] + pc.omega[j1] * rr[j2] - pc.omega[j2] * rr[j1];
+    return (uvec ? amp * uvec[(size_t)i * L.nxyz + r] : 0.0) + pc.vcm[i] + pc.omega[j1] * rr[j2] - pc.omega[j2] * rr[j1];
 }
 
 __device__ __forceinline__ void load_isopoint(const double* __restrict__ acc_n, const double* __restrict__ acc_p,
@@ -236,13 +236,13 @@ __global__ void k_potentials(Lattice L, PhysConst pc, ExtFields ext, const doubl
         const double xi = q ? -1.0 : 1.0;
         double* p = pot[q];
         geff[q][r] = ge[q];
-        p[(size_t)P_U * nx + r] = Uq[q] + (ext.u0[q] ? ext.u0[q][r] : 0.0);
+        p[(size_t)P_U * nx + r] = Uq[q] + (ext.u0[q] ? ext.amp * ext.u0[q][r] : 0.0);
         p[(size_t)P_M * nx + r] = Mq[q];
         for (int i = 0; i < 3; ++i) {
             p[(size_t)(P_W + i) * nx + r] = W[0][i] + xi * W[1][i];                               // Eq. 16
             p[(size_t)(P_S + i) * nx + r] = S[0][i] + xi * S[1][i] - 0.5 * pc.hbarc * pc.omega[i];   // Eq. 17, - omega . s (Eq. 36)
             // Eq. 18; -(1/2)[Uvec . p + p . Uvec] = -i [A . D + D . A] with A = -(hbar c / 2) Uvec (Eqs. 24, 26, 36)
-            p[(size_t)(P_A + i) * nx + r] = A[0][i] + xi * A[1][i] - 0.5 * pc.hbarc * frame_uvec(L, pc, ext.uvec[q], i, r);
+            p[(size_t)(P_A + i) * nx + r] = A[0][i] + xi * A[1][i] - 0.5 * pc.hbarc * frame_uvec(L, pc, ext.uvec[q], ext.amp, i, r);
         }
         p[(size_t)P_DELTA * nx + r] = -ge[q] * kap[q][0];                                         // Eq. 19
         p[(size_t)(P_DELTA + 1) * nx + r] = -ge[q] * kap[q][1];
@@ -333,11 +333,11 @@ __global__ void k_moments1(Lattice L, PhysConst pc, ExtFields ext, const double*
                 v[2 + 3 * q + i] += x[i] * n;
                 v[8 + i] += ji;
                 j2 += ji * ji;
-                v[14] += -pc.hbarc * frame_uvec(L, pc, ext.uvec[q], i, r) * ji - 0.5 * pc.hbarc * pc.omega[i] * d[q][(size_t)(D_S + i) * nx + r];
+                v[14] += -pc.hbarc * frame_uvec(L, pc, ext.uvec[q], ext.amp, i, r) * ji - 0.5 * pc.hbarc * pc.omega[i] * d[q][(size_t)(D_S + i) * nx + r];
             }
             v[11 + q] += hypot(p[q][(size_t)P_DELTA * nx + r], p[q][(size_t)(P_DELTA + 1) * nx + r]) * n;   // Eq. 39
             if (n > 0.0) v[13] += pc.h2m * j2 / n;                                                        // Eq. 40 (B31)
-            if (ext.u0[q]) v[14] += ext.u0[q][r] * n;
+            if (ext.u0[q]) v[14] += ext.amp * ext.u0[q][r] * n;
         }
     }
     block_sums<16>(v, out, L.dV);

@@ -11,6 +11,7 @@
 #include "fft_plane_kernels.cuh"
 #include "grid_kernels.cuh"
 #include "peak_kernels.cuh"
+#include <mutex>
 #include <new>
 #include <stdlib.h>
 #include <vector>
@@ -64,6 +65,8 @@ struct lise_ctx {
     double* ebuf; int eblocks;
     cplx* ovl;
     int R, mma;
+    double amp_now, amp_next;               // amplitudes of the Eq. 24 fields at t_n and t_{n+1} (lise_set_external_amplitudes)
+    int lop_mode;                           // LOP_* requested at creation (lise_create_with_line_operator)
     KernSet ks;
     int have[2], pot_valid;
     long step; double time;
@@ -380,16 +383,22 @@ static KernSet make_v6_set()
 // The DMMA H-apply kernels are instantiated for the lattices the FFT kernels do not cover: 40^3 (BASELINE.json config 4),
 // the paper's 24^2 x 48 and 24^2 x 64 (config 3).  Anything else runs the generic DFMA kernels.
 #define LISE_MMA_SHAPES(X) X(40, 40, 40) X(24, 24, 48) X(24, 24, 64)
-static bool pick_kernels(int nx, int ny, int nz, int R, KernSet* out)
+// mode: LOP_AUTO picks the fastest set instantiated for the lattice; LOP_FFT / LOP_DMMA only that family (false and
+// out->name = nullptr if the lattice has none); LOP_DENSE the generic kernels (lise_create_with_line_operator)
+enum { LOP_AUTO = 0, LOP_FFT = 1, LOP_DMMA = 2, LOP_DENSE = 3 };
+static bool pick_kernels(int nx, int ny, int nz, int R, KernSet* out, int mode = LOP_AUTO)
 {
-    {
+    if (mode == LOP_AUTO || mode == LOP_FFT) {
 #define X(a, b, c_) if (nx == a && ny == b && nz == c_) { *out = make_v6_set<a, b, c_>(); return true; }
         LISE_FFT_SHAPES(X)
 #undef X
+    }
+    if (mode == LOP_AUTO || mode == LOP_DMMA) {
 #define X(a, b, c_) if (nx == a && ny == b && nz == c_) { *out = make_v5_set<a, b, c_>(); return true; }
         LISE_MMA_SHAPES(X)
 #undef X
     }
+    if (mode == LOP_FFT || mode == LOP_DMMA) { out->name = nullptr; return false; }
     if (R == 8) *out = make_set<DenseLines<8>, DenseLines<8>>("dense");
     else if (R == 4) *out = make_set<DenseLines<4>, DenseLines<4>>("dense");
     else *out = make_set<DenseLines<2>, DenseLines<2>>("dense");
@@ -405,16 +414,27 @@ static bool pick_kernels(int nx, int ny, int nz, int R, KernSet* out)
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+// cuTensorMapEncodeTiled through the runtime's driver entry point query (no link against libcuda), resolved once per
+// process under a lock; nullptr if this driver does not provide it (ctx_init then falls back to the generic kernels)
+static EncodeTiledFn resolve_encode_tiled()
+{
+    static std::mutex mu;
+    static int state = 0;                          // 0 not tried, 1 found, -1 missing
+    static EncodeTiledFn encode = nullptr;
+    std::lock_guard<std::mutex> lock(mu);
+    if (state == 0) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qres = cudaDriverEntryPointSymbolNotFound;
+        const cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+        if (e == cudaSuccess && fn && qres == cudaDriverEntryPointSuccess) { encode = (EncodeTiledFn)fn; state = 1; }
+        else { (void)cudaGetLastError(); state = -1; }
+    }
+    return encode;
+}
 static int make_plane_tmap(lise_ctx* c, int kind, const cplx* X, int ncomp, CUtensorMap* out)
 {
-    static EncodeTiledFn encode = nullptr;
-    if (!encode) {
-        void* fn = nullptr;
-        cudaDriverEntryPointQueryResult qres;
-        CK(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
-        if (!fn || qres != cudaDriverEntryPointSuccess) { snprintf(c->err, sizeof(c->err), "cuTensorMapEncodeTiled not available"); return LISE_ECUDA; }
-        encode = (EncodeTiledFn)fn;
-    }
+    const EncodeTiledFn encode = resolve_encode_tiled();
+    if (!encode) { snprintf(c->err, sizeof(c->err), "cuTensorMapEncodeTiled not available"); return LISE_ECUDA; }
     const Lattice& L = c->L;
     const cuuint64_t dims[4] = {(cuuint64_t)2 * L.nz, (cuuint64_t)L.ny, (cuuint64_t)L.nx, (cuuint64_t)(ncomp > 0 ? ncomp : 1)};
     const cuuint64_t strides[3] = {(cuuint64_t)16 * L.nz, (cuuint64_t)16 * L.nz * L.ny, (cuuint64_t)16 * L.nxyz};
@@ -591,12 +611,14 @@ static int coulomb(lise_ctx* c, const double* np)
 }
 
 // potentials of both species from the reduced accumulators acc[0], acc[1]
-static int compute_potentials(lise_ctx* c)
+// amp: amplitude of the external fields of Eq. 24 at the time this Hamiltonian belongs to (lise_set_external_amplitudes)
+static int compute_potentials(lise_ctx* c, double amp)
 {
     const int nx = c->L.nxyz;
     if (c->pc.coulomb) TRY(coulomb(c, c->acc[1] + (size_t)ACC_N * nx));
     k_grid_deriv<<<dim3(nblk(nx, 128), c->njobs1), 128, 0, c->stream>>>(c->L, c->jobs1, c->ctab[0], c->ctab[1], c->ctab[2]); CKL();
     ExtFields ext;
+    ext.amp = amp;
     for (int q = 0; q < 2; ++q) { ext.u0[q] = c->uext[q]; ext.uvec[q] = c->vext[q]; }
     k_potentials<<<nblk(nx, 128), 128, 0, c->stream>>>(c->L, c->pc, ext, c->acc[0], c->acc[1], c->gtmp, c->phi,
                                                         c->dens[0], c->dens[1], c->pot[0], c->pot[1], c->geff[0], c->geff[1]); CKL();
@@ -606,11 +628,11 @@ static int compute_potentials(lise_ctx* c)
 }
 
 // grid-only work between the barriers, timed as one class
-static int grid_phase(lise_ctx* c, int reduce)
+static int grid_phase(lise_ctx* c, int reduce, double amp)
 {
     prof_begin(c, PC_GRID);
     if (reduce) TRY(reduce_all(c));
-    TRY(compute_potentials(c));
+    TRY(compute_potentials(c, amp));
     prof_end(c);
     return LISE_OK;
 }
@@ -618,7 +640,7 @@ static int grid_phase(lise_ctx* c, int reduce)
 static int ensure_potentials(lise_ctx* c)
 {
     if (c->pot_valid) return LISE_OK;
-    TRY(grid_phase(c, 1));
+    TRY(grid_phase(c, 1, c->amp_now));              // the current wavefunctions y_n live at t_n
     c->pot_valid = 1;
     return LISE_OK;
 }
@@ -694,7 +716,7 @@ static int abm_step(lise_ctx* c)
                 if (c->nwf[q] > 0) TRY(dens_accumulate(c, q, S(c, q, RB)));
             }
         }
-        if (phase == 1) TRY(grid_phase(c, 1));     // potentials of the modifier m
+        if (phase == 1) TRY(grid_phase(c, 1, c->amp_next));   // potentials of the modifier m ~ y(t_{n+1}): fields at t_{n+1}
     }
     // y_{n+1} sits in B: A <-> B; f history shifts
     const int ra = c->role[RA]; c->role[RA] = c->role[RB]; c->role[RB] = ra;
@@ -736,7 +758,7 @@ static int starter_step(lise_ctx* c)
     }
     TRY(reduce_all(c));
     for (int q = 0; q < 2; ++q) { k_average<<<nblk(nacc, 256), 256, 0, c->stream>>>(c->acc[q], c->acc0[q], nacc); CKL(); }
-    TRY(compute_potentials(c));                     // H_cor
+    TRY(compute_potentials(c, 0.5 * (c->amp_now + c->amp_next)));   // H_cor: fields averaged like the densities (B33)
     TRY(taylor4_all(c, 0));                         // y_{n+1} -> F
     if (c->par.renormalize) TRY(renormalize_slot(c, RF));
     for (int q = 0; q < 2; ++q) {
@@ -831,7 +853,18 @@ static int ctx_init(lise_ctx* c)
     const size_t nx = L.nxyz;
     // blocking and launch shapes
     c->R = (L.nx % 4 == 0 && L.ny % 4 == 0 && L.nz % 4 == 0) ? 4 : 2;
-    c->mma = pick_kernels(L.nx, L.ny, L.nz, c->R, &c->ks) ? 1 : 0;
+    c->mma = pick_kernels(L.nx, L.ny, L.nz, c->R, &c->ks, c->lop_mode) ? 1 : 0;
+    if (!c->mma && !c->ks.name) {
+        snprintf(c->err, sizeof(c->err), "no %s kernels were instantiated for a %d x %d x %d lattice",
+                 c->lop_mode == LOP_FFT ? "fft" : "dmma", L.nx, L.ny, L.nz);
+        return LISE_EUNSUPPORTED;
+    }
+    // the FFT kernels load their planes through TMA tensor maps: without the driver's encode entry point they cannot
+    // run, so an automatic choice falls back to the generic kernels here, before anything is sized for the set
+    if (c->mma && (c->ks.tma_h[0] || c->ks.tma_h[1]) && !resolve_encode_tiled()) {
+        if (c->lop_mode == LOP_FFT) { snprintf(c->err, sizeof(c->err), "cuTensorMapEncodeTiled not available: the fft kernels cannot run"); return LISE_EUNSUPPORTED; }
+        c->mma = pick_kernels(L.nx, L.ny, L.nz, c->R, &c->ks, LOP_DENSE) ? 1 : 0;
+    }
     if (!c->mma) {
         const int ld = L.nz + 1;
         const int n1[2] = {L.ny, L.nx};
@@ -934,10 +967,12 @@ static int ctx_init(lise_ctx* c)
     return LISE_OK;
 }
 
-static int create_impl(int nx, int ny, int nz, double dx, double dt, int nwf_n, int nwf_p, lise_ctx** out)
+static thread_local char t_create_err[288] = "";   // message of this thread's last failed lise_create (there is no context to ask)
+static int create_impl(int nx, int ny, int nz, double dx, double dt, int nwf_n, int nwf_p, int lop_mode, lise_ctx** out)
 {
     if (!out) return LISE_EINVAL;
     *out = nullptr;
+    t_create_err[0] = 0;
     if (nx < 2 || ny < 2 || nz < 2 || ((nx | ny | nz) & 1) || !(dx > 0.0) || nwf_n < 0 || nwf_p < 0) return LISE_EINVAL;
     if ((long long)nx * ny * nz > (1LL << 26)) return LISE_EUNSUPPORTED;
     lise_ctx* c = new (std::nothrow) lise_ctx();
@@ -954,9 +989,11 @@ static int create_impl(int nx, int ny, int nz, double dx, double dt, int nwf_n, 
     set_physconst(c);
     c->stream = 0;
     c->have[0] = (nwf_n == 0); c->have[1] = (nwf_p == 0);
+    c->lop_mode = lop_mode;
+    c->amp_now = c->amp_next = 1.0;
     int rc = ctx_init(c);
     if (rc != LISE_OK) {
-        fprintf(stderr, "lise_create: %s\n", c->err);
+        snprintf(t_create_err, sizeof(t_create_err), "lise_create: %s", c->err);
         lise_destroy(c);
         return rc;
     }
@@ -965,7 +1002,19 @@ static int create_impl(int nx, int ny, int nz, double dx, double dt, int nwf_n, 
 }
 extern "C" int lise_create(int nx, int ny, int nz, double dx, double dt, int nwf_n, int nwf_p, lise_ctx** out)
 {
-    return guarded([&] { return create_impl(nx, ny, nz, dx, dt, nwf_n, nwf_p, out); });
+    return guarded([&] { return create_impl(nx, ny, nz, dx, dt, nwf_n, nwf_p, LOP_AUTO, out); });
+}
+extern "C" int lise_create_with_line_operator(int nx, int ny, int nz, double dx, double dt, int nwf_n, int nwf_p,
+                                              const char* line_operator, lise_ctx** out)
+{
+    int mode = LOP_AUTO;
+    if (line_operator && strcmp(line_operator, "auto") != 0) {
+        if (!strcmp(line_operator, "fft")) mode = LOP_FFT;
+        else if (!strcmp(line_operator, "dmma")) mode = LOP_DMMA;
+        else if (!strcmp(line_operator, "dense")) mode = LOP_DENSE;
+        else { if (out) *out = nullptr; snprintf(t_create_err, sizeof(t_create_err), "lise_create: unknown line operator \"%.40s\"", line_operator); return LISE_EINVAL; }
+    }
+    return guarded([&] { return create_impl(nx, ny, nz, dx, dt, nwf_n, nwf_p, mode, out); });
 }
 
 extern "C" void lise_destroy(lise_ctx* c)
@@ -1232,6 +1281,14 @@ extern "C" int lise_set_external_fields(lise_ctx* c, int q, const double* u0_dev
     return LISE_OK;
 }
 
+extern "C" int lise_set_external_amplitudes(lise_ctx* c, double f_now, double f_next)
+{
+    if (!c || !(fabs(f_now) < INFINITY) || !(fabs(f_next) < INFINITY)) return LISE_EINVAL;
+    c->amp_now = f_now; c->amp_next = f_next;
+    c->pot_valid = 0;                               // the potentials of y_n carry f_now
+    return LISE_OK;
+}
+
 extern "C" int lise_set_frame(lise_ctx* c, const double* v_cm, const double* omega, const double* origin)
 {
     if (!c) return LISE_EINVAL;
@@ -1248,6 +1305,7 @@ static int observables_ext_impl(lise_ctx* c, lise_observables_ext_t* o)
     TRY(need_both(c));
     TRY(ensure_potentials(c));
     ExtFields ext;
+    ext.amp = c->amp_now;
     for (int q = 0; q < 2; ++q) { ext.u0[q] = c->uext[q]; ext.uvec[q] = c->vext[q]; }
     const int nb = c->eblocks;
     k_moments1<<<nb, 256, 0, c->stream>>>(c->L, c->pc, ext, c->dens[0], c->dens[1], c->pot[0], c->pot[1], c->mbuf); CKL();
@@ -1381,4 +1439,4 @@ extern "C" const char* lise_strerror(int code)
     default: return "unknown error";
     }
 }
-extern "C" const char* lise_last_error(const lise_ctx* c) { return c ? c->err : g_noctx; }
+extern "C" const char* lise_last_error(const lise_ctx* c) { return c ? c->err : (t_create_err[0] ? t_create_err : g_noctx); }

@@ -52,7 +52,8 @@ EXPORTS = ["lise_default_params", "lise_create", "lise_destroy", "lise_set_param
            "lise_densities", "lise_potentials", "lise_apply_h", "lise_step", "lise_observables", "lise_observables_ext",
            "lise_set_time", "lise_boost", "lise_set_external_fields", "lise_set_frame",
            "lise_profile", "lise_profile_read", "lise_measure_fp64_peak", "lise_set_density_group", "lise_line_operator", "lise_line_operator_cost", "lise_line_operator_tables", "lise_launch_count", "lise_device_bytes", "lise_strerror", "lise_last_error",
-           "lise_renormalize_static", "lise_static_last_error"]
+           "lise_renormalize_static", "lise_static_last_error", "lise_create_with_line_operator",
+           "lise_set_external_amplitudes"]
 
 STATIC_MAX_STATES = 16384       # LISE_STATIC_MAX_STATES of include/lise.h
 
@@ -86,6 +87,7 @@ def load():
     vp, ip, dp = C.c_void_p, C.c_int, C.c_double
     lib.lise_default_params.argtypes = [C.POINTER(Params)]
     lib.lise_create.argtypes = [ip, ip, ip, dp, dp, ip, ip, C.POINTER(vp)]
+    lib.lise_create_with_line_operator.argtypes = [ip, ip, ip, dp, dp, ip, ip, C.c_char_p, C.POINTER(vp)]
     lib.lise_destroy.argtypes = [vp]; lib.lise_destroy.restype = None
     lib.lise_set_params.argtypes = [vp, C.POINTER(Params)]
     lib.lise_set_stream.argtypes = [vp, vp]
@@ -107,6 +109,7 @@ def load():
     lib.lise_boost.argtypes = [vp, ip, vp]
     lib.lise_set_external_fields.argtypes = [vp, ip, vp, vp]
     lib.lise_set_frame.argtypes = [vp, C.POINTER(dp), C.POINTER(dp), C.POINTER(dp)]
+    lib.lise_set_external_amplitudes.argtypes = [vp, dp, dp]
     lib.lise_profile.argtypes = [vp, ip]
     lib.lise_profile_read.argtypes = [vp, C.POINTER(dp), C.POINTER(C.c_long)]
     lib.lise_measure_fp64_peak.argtypes = [vp, dp, C.POINTER(dp), C.POINTER(dp)]
@@ -213,7 +216,7 @@ class LiseError(RuntimeError):
 class Lise:
     """One TDSLDA context on the current CUDA device.  Tensors are torch CUDA tensors (complex128 / float64)."""
 
-    def __init__(self, nx, ny, nz, dx, dt, nwf_n, nwf_p, params=None, stream=None, device=None):
+    def __init__(self, nx, ny, nz, dx, dt, nwf_n, nwf_p, params=None, stream=None, device=None, line_operator=None):
         if not torch.cuda.is_available():
             raise LiseError("no CUDA device: the TDSLDA path has no CPU fallback")
         self.lib = load()
@@ -224,10 +227,13 @@ class Lise:
         self.dx, self.dt = dx, dt
         self._h = C.c_void_p()
         with torch.cuda.device(self.device):
-            rc = self.lib.lise_create(nx, ny, nz, dx, dt, nwf_n, nwf_p, C.byref(self._h))
+            if line_operator is None:
+                rc = self.lib.lise_create(nx, ny, nz, dx, dt, nwf_n, nwf_p, C.byref(self._h))
+            else:       # "fft" | "dmma" | "dense" | "auto": lise_create_with_line_operator
+                rc = self.lib.lise_create_with_line_operator(nx, ny, nz, dx, dt, nwf_n, nwf_p, line_operator.encode(), C.byref(self._h))
         if rc != 0:
             self._h = C.c_void_p()
-            raise LiseError(f"lise_create failed: {self.lib.lise_strerror(rc).decode()} ({rc})")
+            raise LiseError(f"lise_create failed: {self.lib.lise_strerror(rc).decode()} ({rc}) {self.lib.lise_last_error(None).decode()}")
         st = torch.cuda.current_stream(self.device) if stream is None else stream
         self._stream_ptr = st.cuda_stream
         self._chk(self.lib.lise_set_stream(self._h, C.c_void_p(st.cuda_stream)), "lise_set_stream")
@@ -374,6 +380,10 @@ class Lise:
         a = C.c_void_p() if u0 is None else self._dev(u0, torch.float64, self.nxyz)
         b = C.c_void_p() if uvec is None else self._dev(uvec, torch.float64, 3 * self.nxyz)
         self._chk(self.lib.lise_set_external_fields(self._h, q, a, b), "lise_set_external_fields")
+
+    def set_external_amplitudes(self, f_now, f_next):
+        """f(t_n), f(t_n + dt) on the profiles of set_external_fields; call before every step(1) of a driven run."""
+        self._chk(self.lib.lise_set_external_amplitudes(self._h, float(f_now), float(f_next)), "lise_set_external_amplitudes")
 
     def set_frame(self, v_cm=(0.0, 0.0, 0.0), omega=(0.0, 0.0, 0.0), origin=(0.0, 0.0, 0.0)):
         arrs = [(C.c_double * 3)(*[float(x) for x in v]) for v in (v_cm, omega, origin)]

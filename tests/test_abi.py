@@ -37,6 +37,11 @@ def test_calls_without_gpu_fail_cleanly():
     for code in (0, -1, -2, -3, -4, -5, -99):
         assert len(lib.lise_strerror(code)) > 0
     assert lib.lise_default_params(None) == -1
+    # an unknown line operator is refused before any CUDA call, and the message is kept for the calling thread
+    import ctypes
+    h = ctypes.c_void_p(1)
+    assert lib.lise_create_with_line_operator(8, 8, 8, 1.0, 0.05, 1, 0, b"cufft", ctypes.byref(h)) == -1
+    assert h.value is None and b"unknown line operator" in lib.lise_last_error(None)
 
 
 def test_product_path_does_not_import_oracle():

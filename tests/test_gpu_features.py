@@ -173,6 +173,40 @@ def test_boost_external_fields_and_frames():
     gc.close(); oc.close()
 
 
+def test_driven_external_fields_with_amplitude_pairs():
+    """U0(r) f(t), Uvec(r) f(t) with (f(t_n), f(t_{n+1})) set before every step: 3 starter + 4 ABM steps,
+    potentials and e_ext at an amplitude other than 1, against the oracle (whose driven stepping is pinned to the closed
+    form of a driven free state)."""
+    shape, nwf = (12, 12, 16), (8, 6)
+    cfg, psi, oc, gc = _pair(shape, nwf, seed=38, cfg_idx=0)
+    x = np.meshgrid(*[np.arange(n) * cfg["dx"] for n in shape], indexing="ij")
+    L = [n * cfg["dx"] for n in shape]
+    for q in (0, 1):
+        u0 = 6.0 * np.cos(2 * np.pi * x[2] / L[2]) * (1 + q) + 3.0
+        uv = 0.01 * np.stack([np.cos(2 * np.pi * x[(i + 2) % 3] / L[(i + 2) % 3] + q) for i in range(3)])
+        oc.set_external_fields(q, u0=u0, uvec=uv)
+        gc.set_external_fields(q, u0=torch.from_numpy(u0).cuda(), uvec=torch.from_numpy(np.ascontiguousarray(uv)).cuda())
+    f = lambda t: np.cos(2.0 * t) + 0.5 * t
+    dt = cfg["dt"]
+    for i in range(7):
+        for c in (oc, gc):
+            c.set_external_amplitudes(f(i * dt), f((i + 1) * dt))
+            c.step(1)
+    for c in (oc, gc):
+        c.set_external_amplitudes(f(7 * dt), f(8 * dt))
+    _compare_state(oc, gc, nwf, "driven, after 7 steps")
+    _compare_ext(oc, gc, "driven external terms")
+    # the run really was driven: a static field (amplitudes 1, 1 throughout) ends elsewhere
+    cfg2, psi2, oc2, gc2 = _pair(shape, nwf, seed=38, cfg_idx=0)
+    oc2.close()
+    for q in (0, 1):
+        u0 = 6.0 * np.cos(2 * np.pi * x[2] / L[2]) * (1 + q) + 3.0
+        gc2.set_external_fields(q, u0=torch.from_numpy(u0).cuda())
+    gc2.step(7)
+    assert rel(gc2.get_wavefunctions(0).cpu().numpy(), gc.get_wavefunctions(0).cpu().numpy()) > 1e-6
+    gc2.close(); gc.close(); oc.close()
+
+
 def test_static_solution_stays_stationary_on_the_gpu():
     """A self-consistent Hartree-Fock state (built on the CPU by dense diagonalisation in the oracle's mean field,
     tests/dense_ref.py; pairing off, Coulomb on, 2 + 2 particles on 8^3: the FFT H-apply kernels) is a fixed point of the

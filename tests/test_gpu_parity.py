@@ -51,9 +51,13 @@ CASES = {
     # the multi-chunk pipeline: 7 + 4 chunks with ragged tails, double-buffered W / eta, update on the second stream,
     # density launches per group of 3 chunks (a species change inside a group)
     "c1_24c_pipeline": (1, None, None, (40, 24), 10, dict(chunk=6, dgroup=3, overlap=True)),
-    "c2_32c": (2, None, None, (64, 64), 10, None),
-    "c3_24x24x64": (3, None, None, (64, 64), 10, None),
-    "c4_40c": (4, None, None, (64, 64), 10, None),
+    # configs 2-4 in the schedule bench.py times as well: three chunks per species with a ragged tail (96 + 96 + 64,
+    # 48 + 48 + 32), double-buffered W, update on the second stream, densities per group of 2 chunks.  32^3 (a target
+    # workload) at SURVEY 8(c)'s 256 + 256 states; the two long-line lattices at 128 + 128, because the oracle's share of
+    # these three cases (about 7 minutes on the box's 16 cores) has to fit the 20 minutes the whole GPU suite is given
+    "c2_32c": (2, None, None, (256, 256), 10, dict(chunk=96, dgroup=2, overlap=True)),
+    "c3_24x24x64": (3, None, None, (128, 128), 10, dict(chunk=48, dgroup=2, overlap=True)),
+    "c4_40c": (4, None, None, (128, 128), 10, dict(chunk=48, dgroup=2, overlap=True)),
     # the paper's own fission box 24^2 x 48 (L1076): 48-point lines = 8 x 6, the size-6 real DFT of the DMMA line operator
     "p_24x24x48": (3, (24, 24, 48), None, (12, 8), 5, None),
 }
@@ -383,4 +387,136 @@ def test_defects_of_a_non_orthonormal_set():
     o = g.observables()
     assert abs(o["norm_defect"] - (scale ** 2 - 1.0)) < 1e-12
     assert abs(o["ortho_defect"] - math.sin(theta)) < 1e-12
+    g.close()
+
+
+def _white_noise_states(shape, dx, nwf, seed):
+    """every component of every state drawn from uniform(-1, 1) + i uniform(-1, 1) at every lattice point
+    (then normalised to dV sum |psi|^2 = 1): all wavevectors up to and including the Nyquist planes carry full weight."""
+    rng = np.random.default_rng(seed)
+    psi = rng.uniform(-1.0, 1.0, (nwf, 4) + tuple(shape)) + 1j * rng.uniform(-1.0, 1.0, (nwf, 4) + tuple(shape))
+    psi /= np.sqrt((np.abs(psi) ** 2).sum(axis=(1, 2, 3, 4), keepdims=True) * dx ** 3)
+    return np.ascontiguousarray(psi)
+
+
+# one lattice per kernel family: whole-state FFT units (24^3), 2-spinor FFT units with the pairing block in the xz
+# kernel (32^3), block-diagonalised circulant on the fp64 tensor cores (24^2 x 48), generic DFMA kernels (6 x 10 x 12)
+@pytest.mark.parametrize("shape,line_op", [((24, 24, 24), "fft"), ((32, 32, 32), "fft"), ((24, 24, 48), "dmma"), ((6, 10, 12), "dense")])
+def test_white_noise_states_reach_the_nyquist_branch_of_every_kernel_family(shape, line_op):
+    """The band-limited generator of the other cases feeds the Nyquist planes (D zeroed, D2 kept) only
+    through the envelope's leakage; white noise (the paper's own noise distribution, L685) puts full weight there.
+    lise_densities, lise_potentials and lise_apply_h of such states against the oracle, in every kernel family."""
+    from paper_2009_00745_b200 import lise
+    dx, nwf = 1.25, (6, 4)
+    psi = [_white_noise_states(shape, dx, nwf[q], 685 + q) for q in (0, 1)]
+    oc = ref.RefContext(*shape, dx, 0.05, *nwf)
+    gc = lise.Lise(*shape, dx, 0.05, *nwf)
+    assert gc.line_operator() == line_op
+    for q in (0, 1):
+        oc.set_wavefunctions(q, psi[q]); gc.set_wavefunctions(q, torch.from_numpy(psi[q]).cuda())
+    for q in (0, 1):
+        assert field_rel(gc.densities(q).cpu().numpy(), oc.densities(q)) < TOL_DENS, (shape, "densities", q)
+        assert field_rel(gc.potentials(q).cpu().numpy(), oc.potentials(q)) < 1e-10, (shape, "potentials", q)
+        h_ref = oc.apply_h(q, psi[q])
+        h_gpu = gc.apply_h(q, torch.from_numpy(psi[q]).cuda()).cpu().numpy()
+        assert rel(h_gpu, h_ref.reshape(h_gpu.shape)) < 1e-12, (shape, "H psi", q)
+    gc.close(); oc.close()
+
+
+def test_line_operator_families_agree_and_can_be_chosen_at_creation():
+    """lise_create_with_line_operator: the generic DFMA kernels against the FFT kernels on 24^3 (densities, potentials,
+    H psi, 3 starter + 1 ABM steps) and against the tensor-core kernels on 24^2 x 48 (H psi); families that were not
+    instantiated for a lattice, and unknown names, are refused with a message."""
+    from paper_2009_00745_b200 import lise
+    cfg = dict(inputs.CONFIGS[1])
+    nwf = (12, 8)
+    psi = [inputs.make_species(cfg, q, nwf[q], seed=77).cuda() for q in (0, 1)]
+    ctx = {}
+    for name in ("fft", "dense"):
+        g = lise.Lise(*cfg["shape"], cfg["dx"], cfg["dt"], *nwf, line_operator=name)
+        assert g.line_operator() == name
+        for q in (0, 1):
+            g.set_wavefunctions(q, psi[q])
+        ctx[name] = g
+    a, b = ctx["fft"], ctx["dense"]
+    for q in (0, 1):
+        assert field_rel(a.densities(q).cpu().numpy(), b.densities(q).cpu().numpy()) < TOL_DENS
+        assert field_rel(a.potentials(q).cpu().numpy(), b.potentials(q).cpu().numpy()) < 1e-10
+        assert rel(a.apply_h(q, psi[q]).cpu().numpy(), b.apply_h(q, psi[q]).cpu().numpy()) < 1e-12
+    a.step(4); b.step(4)
+    for q in (0, 1):
+        assert rel(a.get_wavefunctions(q).cpu().numpy(), b.get_wavefunctions(q).cpu().numpy()) < TOL_WF
+    ea, eb = a.observables()["energy"], b.observables()["energy"]
+    assert abs(ea - eb) < TOL_E * abs(eb)
+    a.close(); b.close()
+    shape = (24, 24, 48)
+    cfg3 = dict(inputs.CONFIGS[3]); cfg3["shape"] = shape
+    psi3 = [inputs.make_species(cfg3, q, 5, seed=78).cuda() for q in (0, 1)]
+    out = {}
+    for name in ("dmma", "dense"):
+        g = lise.Lise(*shape, cfg3["dx"], cfg3["dt"], 5, 5, line_operator=name)
+        assert g.line_operator() == name
+        for q in (0, 1):
+            g.set_wavefunctions(q, psi3[q])
+        out[name] = [g.apply_h(q, psi3[q]).cpu().numpy() for q in (0, 1)]
+        g.close()
+    for q in (0, 1):
+        assert rel(out["dmma"][q], out["dense"][q]) < 1e-12
+    with pytest.raises(lise.LiseError, match="no dmma kernels"):
+        lise.Lise(24, 24, 24, 1.25, 0.05, 2, 2, line_operator="dmma")
+    with pytest.raises(lise.LiseError, match="no fft kernels"):
+        lise.Lise(6, 10, 12, 1.25, 0.05, 2, 2, line_operator="fft")
+    with pytest.raises(lise.LiseError, match="unknown line operator"):
+        lise.Lise(24, 24, 24, 1.25, 0.05, 2, 2, line_operator="cufft")
+    g = lise.Lise(24, 24, 24, 1.25, 0.05, 2, 2, line_operator="auto")
+    assert g.line_operator() == "fft"
+    g.close()
+
+
+@pytest.mark.parametrize("shape", [(24, 24, 24), (32, 32, 32), (24, 24, 48), (6, 10, 12)])
+def test_caller_buffers_are_not_overrun(shape):
+    """compute-sanitizer is closed on this GPU pool (profiles/r3_sanitizer.md), so the bounds of the caller-owned buffers
+    are checked here instead: every output of the C ABI is a window inside a larger allocation filled with a canary, the
+    inputs sit between canaries too, and after lise_densities / lise_potentials / lise_apply_h / lise_step /
+    lise_get_wavefunctions on a ragged state count the canaries on both sides must be untouched -- for each kernel
+    family (FFT whole-state, FFT 2-spinor, tensor-core, generic)."""
+    from paper_2009_00745_b200 import lise
+    cfg = dict(inputs.CONFIGS[1]); cfg["shape"] = shape
+    nwf, nxyz, pad = (7, 5), int(np.prod(shape)), 4096
+    CAN = complex(-7.25e300, 3.5e299)
+
+    def window(count, dtype):
+        big = torch.full((count + 2 * pad,), CAN if dtype == torch.complex128 else CAN.real, dtype=dtype, device="cuda")
+        return big, big[pad:pad + count]
+
+    def intact(big, count):
+        edge = torch.cat([big[:pad], big[pad + count:]])
+        want = CAN if big.dtype == torch.complex128 else CAN.real
+        return bool((edge == want).all())
+
+    g = lise.Lise(*shape, cfg["dx"], cfg["dt"], *nwf)
+    g.set_chunk(3)                                                  # ragged: 3 + 3 + 1 and 3 + 2 states
+    for q in (0, 1):
+        n = nwf[q] * 4 * nxyz
+        big_in, w_in = window(n, torch.complex128)
+        w_in.copy_(inputs.make_species(cfg, q, nwf[q], seed=90).reshape(-1).cuda())
+        g.set_wavefunctions(q, w_in.reshape((nwf[q], 4) + shape))
+        assert intact(big_in, n)
+    g.step(4)                                                       # 3 starter + 1 ABM step on the internal buffers
+    for q in (0, 1):
+        n = nwf[q] * 4 * nxyz
+        for call in (g.densities, g.potentials):
+            big, w = window(14 * nxyz, torch.float64)
+            call(q, out=w.reshape((14,) + shape))
+            torch.cuda.synchronize()
+            assert intact(big, 14 * nxyz) and bool(torch.isfinite(w).all()), (call.__name__, q)
+        big_o, w_o = window(n, torch.complex128)
+        g.get_wavefunctions(q, out=w_o.reshape((nwf[q], 4) + shape))
+        big_h, w_h = window(n, torch.complex128)
+        g.apply_h(q, w_o, out=w_h)
+        torch.cuda.synchronize()
+        assert intact(big_o, n) and intact(big_h, n), q
+        assert bool(torch.isfinite(w_h.real).all()) and float(w_h.abs().max()) < 1e6
+    o = g.observables()
+    assert o["norm_defect"] < 1e-10 and np.isfinite(o["energy"])
     g.close()
